@@ -1,0 +1,169 @@
+/* grmhd.h -- C ABI of libgrmhd.so: the B200 (sm_100a) fp64 GRMHD substep library.
+ *
+ * What it computes: the Valencia-formulation GRMHD right-hand side and Runge-Kutta
+ * substep of AsterX (arXiv 2406.11669; PAPER.md) on ONE uniform 3-D Cartesian block
+ * with the spacetime metric held fixed:
+ *   conservative->primitive recovery (eqs 36-41; atmosphere PAPER.md:326),
+ *   minmod / PPM face reconstruction,
+ *   HLLE fluxes in x,y,z (eq. 29; state/flux vectors eq. 18),
+ *   flux divergence + metric sources (eqs 17,19),
+ *   staggered vector-potential update with flux-CT electric field, B = curl A
+ *   (algebraic gauge PAPER.md:159),
+ *   RK2/RK3/RK4 stage combination and
+ *   a max-characteristic-speed reduction for the CFL time step.
+ * The ADM variables alpha, beta^i, gamma_ij, K_ij are INPUT fields.
+ * DESIGN.md lists every reading of the paper (R/G rows) this library implements.
+ *
+ * Memory model
+ *   - Every pointer argument marked [dev|host] may be a CUDA device pointer or a host
+ *     pointer (pinned host memory recommended); the library copies with
+ *     cudaMemcpyDefault (unified virtual addressing decides the direction).
+ *   - The caller owns every buffer, including the workspace (device memory, e.g. a
+ *     torch tensor).  The library never allocates device memory for fields; it carves its
+ *     structure-of-arrays state out of the workspace.  The workspace must stay alive and
+ *     untouched until grmhd_destroy.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  All work of a
+ *     handle is enqueued on that one stream.  Handles are not thread-safe.
+ *
+ * Array layout (all fp64, C order, x fastest), g = ghosts (must be 3):
+ *   cell-centred arrays : shape (nz+2g, ny+2g, nx+2g); cell (i,j,k), i in [-g, nx+g), is at
+ *                         linear index ((k+g)*(ny+2g) + (j+g))*(nx+2g) + (i+g);
+ *                         centre x_i = x_0 + (i+1/2) dx.
+ *   staggered arrays    : shape (nz+2g+1, ny+2g+1, nx+2g+1), LOWER convention:
+ *                         A_x[i,j,k] at (i, j-1/2, k-1/2); A_y at (i-1/2, j, k-1/2);
+ *                         A_z at (i-1/2, j-1/2, k)     (Fig. 1).
+ *
+ * Errors: every call returns GRMHD_OK (0) or a negative code; no exceptions, aborts or
+ * stdout.  grmhd_last_error gives a human-readable string for the last failure.
+ * Per-cell con2prim failures are not errors; they are counted (grmhd_get_stats).
+ */
+#ifndef GRMHD_H
+#define GRMHD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GRMHD_OK        0
+#define GRMHD_EINVAL   -1  /* bad size / NULL pointer / ghosts != 3 / bad option        */
+#define GRMHD_ENOMEM   -2  /* workspace too small                                      */
+#define GRMHD_ESTATE   -3  /* call order: step before metric+prims, vecpot before prims */
+#define GRMHD_ECUDA    -4  /* CUDA runtime error (string in grmhd_last_error)          */
+#define GRMHD_ENUMERIC -5  /* dt came out NaN / non-positive / infinite                */
+
+typedef struct grmhd grmhd; /* opaque handle (host memory, owned by the library) */
+
+/* Options.  EOS: ideal fluid p=(Gamma-1) rho eps (eq. 46); the atmosphere
+ * uses the polytrope p=K rho^Gamma_p (eqs 47-48). */
+typedef struct {
+  double gamma_ad;   /* ideal-fluid adiabatic index Gamma, eq. (46)                        */
+  double poly_k;     /* atmosphere polytropic constant K, eq. (47)                         */
+  double poly_gamma; /* atmosphere polytropic exponent, eq. (47)                           */
+  double rho_atm;    /* rest-mass density floor rho_atm                     */
+  double p_floor;    /* pressure floor, > 0                                                */
+  double w_max;      /* Lorentz-factor cap (paper silent; G20), e.g. 100         */
+  double c2p_tol;    /* Newton stop: |dz|/z + |dv2| < c2p_tol (G18), e.g. 1e-12  */
+  int    c2p_maxit;  /* Newton iteration cap, e.g. 100                                     */
+  int    recon;      /* 0 = minmod, 1 = PPM                                 */
+  int    ppm_flatten;/* 1 = PPM shock flattening on (G8)                         */
+  int    riemann;    /* 0 = HLLE eq. (29); 1 = Lax-Friedrichs eq. (30)                     */
+  int    rk;         /* 2 = SSP-RK2, 3 = SSP-RK3, 4 = classic RK4 (G15)          */
+  int    bc[3];      /* per axis x,y,z: 0 = periodic, 1 = outflow           */
+} grmhd_opts;
+
+typedef struct {
+  double t;             /* simulation time reached                                         */
+  double dt;            /* last time step used                                             */
+  double maxspeed[3];   /* max |lambda| per direction of the CURRENT primitives (A8)       */
+  long long steps;      /* full RK steps taken                                             */
+  long long c2p_fail;   /* cell-substeps reset to atmosphere after a failed Newton solve   */
+  long long p_fix;      /* cell-substeps whose pressure was raised to p_floor              */
+  long long atmo;       /* cell-substeps reset because D <= rho_atm or masked              */
+  long long w_cap;      /* cell-substeps whose velocity was rescaled to w_max              */
+  long long c2p_maxiter;/* largest Newton iteration count seen                             */
+} grmhd_stats;
+
+/* Bytes of DEVICE workspace the handle needs for this block (0 on invalid arguments). */
+size_t grmhd_workspace_bytes(int nx, int ny, int nz, int ghosts, const grmhd_opts* opts);
+
+/* Create a handle.  dx[3]: host array of cell sizes.  workspace: [dev] pointer, at least
+ * grmhd_workspace_bytes() bytes, 256-byte aligned.  stream: cudaStream_t or NULL.
+ * Errors: EINVAL (nx,ny,nz < 1, < 2 on an outflow axis, ghosts != 3, dx <= 0, bad opts),
+ * ENOMEM (workspace too small), ECUDA. */
+int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3],
+                 const grmhd_opts* opts, void* workspace, size_t workspace_bytes,
+                 void* stream, grmhd** out);
+int grmhd_destroy(grmhd* h);
+
+/* 16 cell-centred padded arrays [dev|host], ghosts SUPPLIED BY THE CALLER, in the order
+ * alpha, betax, betay, betaz, gxx, gxy, gxz, gyy, gyz, gzz, kxx, kxy, kxz, kyy, kyz, kzz
+ * (ADM variables).  field: host array of 16 pointers. */
+int grmhd_set_metric(grmhd* h, const double* const field[16]);
+
+/* 8 cell-centred padded arrays [dev|host]: rho, vx, vy, vz (Eulerian v^i), press,
+ * Bx, By, Bz (Eulerian B^i; the three B pointers may all be NULL = no static field).
+ * Fills ghosts by the boundary condition, builds the static densitised face field B~0
+ * (G16), zeroes A_i, and initialises the conserved variables by eqs (20)-(22)
+ * (PAPER.md:379).  Requires set_metric first (ESTATE). */
+int grmhd_set_prims(grmhd* h, const double* const field[8]);
+
+/* 3 staggered arrays [dev|host] A_x, A_y, A_z; total field B~ = B~0 + curl A (eq. 24,
+ * PAPER.md:149).  Requires set_prims first (ESTATE); re-initialises the conserved
+ * variables with the new field. */
+int grmhd_set_vecpot(grmhd* h, const double* const field[3]);
+
+/* Optional cell-centred padded uint8 array [dev|host]; cells with mask != 0 are reset to
+ * atmosphere at every con2prim (excision floor, BASELINE config 3).  NULL clears it. */
+int grmhd_set_mask(grmhd* h, const unsigned char* mask);
+
+/* n full RK steps; dt = cfl * min_d dx_d / maxspeed_d from the primitives at the start of
+ * each step (or the "fixed_dt" option).  Asynchronous: returns after enqueue. */
+int grmhd_step(grmhd* h, int n, double cfl);
+
+/* Steps until t >= t_end, clipping the last dt; synchronises once per step.
+ * nsteps_done may be NULL. */
+int grmhd_step_until(grmhd* h, double t_end, double cfl, int* nsteps_done);
+
+/* Outputs [dev|host]; each synchronises the stream before returning.
+ * get_prims: 8 padded cell-centred arrays incl. filled ghosts (rho,v^i,p,B^i centred).
+ * get_cons : 8 padded cell-centred arrays, UNdensitised D, S_x, S_y, S_z, tau, B^x, B^y, B^z;
+ *            interior cells only, ghost cells are set to 0.
+ * get_vecpot: 3 staggered arrays incl. filled ghosts. */
+int grmhd_get_prims(grmhd* h, double* const field[8]);
+int grmhd_get_cons(grmhd* h, double* const field[8]);
+int grmhd_get_vecpot(grmhd* h, double* const field[3]);
+
+/* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off).
+ * Unknown key -> EINVAL. */
+int grmhd_set_option(grmhd* h, const char* key, double value);
+
+/* Synchronises and copies the counters.  Returns ENUMERIC if any dt was not finite/positive. */
+int grmhd_get_stats(grmhd* h, grmhd_stats* out);
+
+/* Number of kernels this handle has launched so far (host-side counter). */
+long long grmhd_launch_count(const grmhd* h);
+
+const char* grmhd_last_error(const grmhd* h);
+
+/* ---- stand-alone kernels exposed for unit parity tests and micro-benchmarks ---------
+ * Pointwise batches on plain [dev] arrays of n states, structure-of-arrays, each array n long.
+ * prim: 8 arrays rho,vx,vy,vz,p,Bx,By,Bz; metric: 10 arrays alpha,beta^i(3),gamma_ij(6);
+ * cons: 8 arrays UNdensitised D,S_x,S_y,S_z,tau,B^x,B^y,B^z. */
+int grmhd_prim2con_batch(const double* const prim[8], const double* const metric[10],
+                         double* const cons[8], long long n, const grmhd_opts* opts,
+                         void* stream);
+/* cons in (5 hydro rows + 3 B rows) -> prim out (5), status out (int32 per state: bit0
+ * atmosphere, bit1 c2p failure, bit2 pressure fix, bit3 W cap), iterations (int32). */
+int grmhd_con2prim_batch(const double* const cons[8], const double* const metric[10],
+                         double* const prim[5], int* status, int* iters, long long n,
+                         const grmhd_opts* opts, void* stream);
+/* Dependent-free DFMA loop used to MEASURE the FP64 pipe peak: each of `threads` threads
+ * performs `iters` * 16 DFMAs; out receives one double per thread.  */
+int grmhd_dfma_peak(double* out, long long threads, int iters, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRMHD_H */
