@@ -1,0 +1,542 @@
+// grmhd.cu -- C ABI of libgrmhd.so (include/grmhd.h): host-side step driver that only
+// enqueues kernels on the handle's stream; every numerical step runs in the CUDA kernels of
+// kernels_*.cuh.  There is no CPU fallback: without a CUDA device every compute call
+// returns GRMHD_ECUDA.
+#include "../../include/grmhd.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "kernels_flux.cuh"
+#include "kernels_batch.cuh"
+
+using namespace gk;
+
+struct grmhd {
+  Geom g;
+  Eos E;
+  grmhd_opts o;
+  double* base = nullptr;
+  double* stage = nullptr;
+  unsigned char* mask = nullptr;
+  DevState* dst = nullptr;
+  cudaStream_t s = nullptr;
+  int nfields = 0;
+  long long stage_elems = 0;
+  bool have_metric = false, have_prims = false, have_mask = false;
+  double cfl_set = -1.0, fixed_dt = 0.0, fixed_set = -1.0, tend_set = -2.0;
+  long long steps = 0;
+  long long launches = 0;
+  char err[256] = {0};
+};
+
+namespace {
+
+int fail(grmhd* h, int code, const char* msg) {
+  if (h) snprintf(h->err, sizeof h->err, "%s", msg);
+  return code;
+}
+
+int cuda_fail(grmhd* h, cudaError_t e, const char* where) {
+  if (h) snprintf(h->err, sizeof h->err, "%s: %s", where, cudaGetErrorString(e));
+  return GRMHD_ECUDA;
+}
+
+#define CK(call)                                                     \
+  do {                                                               \
+    cudaError_t e_ = (call);                                         \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, #call);           \
+  } while (0)
+
+#define CKL(name)                                                    \
+  do {                                                               \
+    h->launches++;                                                   \
+    cudaError_t e_ = cudaGetLastError();                             \
+    if (e_ != cudaSuccess) return cuda_fail(h, e_, name);            \
+  } while (0)
+
+bool valid_opts(const grmhd_opts* o) {
+  if (!o) return false;
+  for (int a = 0; a < 3; a++)
+    if (o->bc[a] != 0 && o->bc[a] != 1) return false;
+  return o->rk >= 2 && o->rk <= 4 && o->recon >= 0 && o->recon <= 1 && o->gamma_ad > 1.0 &&
+         o->p_floor > 0 && o->rho_atm > 0 && o->w_max > 1.0 && o->c2p_maxit >= 1 &&
+         o->riemann >= 0 && o->riemann <= 1;
+}
+
+Eos make_eos(const grmhd_opts& o) {
+  Eos E;
+  E.Gamma = o.gamma_ad;
+  E.GoGm1 = o.gamma_ad / (o.gamma_ad - 1.0);
+  E.gm1oG = (o.gamma_ad - 1.0) / o.gamma_ad;
+  E.rho_atm = o.rho_atm;
+  E.p_atm = std::fmax(o.poly_k * std::pow(o.rho_atm, o.poly_gamma), o.p_floor);
+  E.p_floor = o.p_floor;
+  E.v2max = 1.0 - 1.0 / (o.w_max * o.w_max);
+  E.c2p_tol = o.c2p_tol;
+  E.c2p_maxit = o.c2p_maxit;
+  E.recon = o.recon;
+  E.flatten = o.ppm_flatten;
+  E.riemann = o.riemann;
+  return E;
+}
+
+bool make_geom(int nx, int ny, int nz, const double dx[3], const grmhd_opts* o, Geom* g) {
+  if (nx < 1 || ny < 1 || nz < 1) return false;
+  g->nx = nx; g->ny = ny; g->nz = nz;
+  g->PXP = ((nx + 8 + 3) / 4) * 4;
+  g->PY = ny + 2 * G + 1;
+  g->PZ = nz + 2 * G + 1;
+  g->sy = g->PXP;
+  g->sz = (long long)g->PXP * g->PY;
+  g->NP = g->sz * g->PZ;
+  g->NPA = ((g->NP + 31) / 32) * 32;
+  for (int a = 0; a < 3; a++) {
+    g->dx[a] = dx ? dx[a] : 1.0;
+    g->idx[a] = 1.0 / g->dx[a];
+    g->bc[a] = o ? o->bc[a] : 0;
+  }
+  return true;
+}
+
+long long stage_elems_of(const Geom& g) {
+  const long long n = (long long)(g.nx + 2 * G + 1) * (g.ny + 2 * G + 1) * (g.nz + 2 * G + 1);
+  return ((n + 31) / 32) * 32;
+}
+
+int nfields_of(const grmhd_opts* o) { return o->rk == 4 ? F_END_RK4 : F_END_RK23; }
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+dim3 blk3() { return dim3(32, 4, 1); }
+dim3 grd3(int ex, int ey, int ez) { return dim3((ex + 31) / 32, (ey + 3) / 4, ez); }
+int grd1(long long n) {
+  long long b = (n + 255) / 256;
+  return (int)(b > 65535 * 16 ? 65535 * 16 : (b < 1 ? 1 : b));
+}
+
+// external array -> internal field (through the staging buffer when the source is host memory)
+int copy_in(grmhd* h, const double* src, int id, bool stag) {
+  const Geom& g = h->g;
+  const int ex = g.nx + 2 * G + stag, ey = g.ny + 2 * G + stag, ez = g.nz + 2 * G + stag;
+  const long long n = (long long)ex * ey * ez;
+  const double* dsrc = src;
+  if (!is_device_ptr(src)) {
+    CK(cudaMemcpyAsync(h->stage, src, n * sizeof(double), cudaMemcpyDefault, h->s));
+    dsrc = h->stage;
+  }
+  k_repack_in<<<grd1(n), 256, 0, h->s>>>(dsrc, h->base + (size_t)id * g.NPA, g, ex, ey, ez);
+  CKL("k_repack_in");
+  return GRMHD_OK;
+}
+
+int copy_out(grmhd* h, int id, double* dst, bool stag, int mode) {
+  const Geom& g = h->g;
+  const int ex = g.nx + 2 * G + stag, ey = g.ny + 2 * G + stag, ez = g.nz + 2 * G + stag;
+  const long long n = (long long)ex * ey * ez;
+  const bool dev = is_device_ptr(dst);
+  double* ddst = dev ? dst : h->stage;
+  k_repack_out<<<grd1(n), 256, 0, h->s>>>(h->base + (size_t)id * g.NPA, ddst, h->base, g, ex,
+                                          ey, ez, mode);
+  CKL("k_repack_out");
+  if (!dev) CK(cudaMemcpyAsync(dst, h->stage, n * sizeof(double), cudaMemcpyDefault, h->s));
+  return GRMHD_OK;
+}
+
+int zero_field(grmhd* h, int id) {
+  k_fill_zero<<<grd1(h->g.NPA), 256, 0, h->s>>>(h->base + (size_t)id * h->g.NPA, h->g.NPA);
+  CKL("k_fill_zero");
+  return GRMHD_OK;
+}
+
+// R15: x, then y, then z pass
+int fill_ghosts(grmhd* h, const FillArgs& fa) {
+  const Geom& g = h->g;
+  for (int a = 0; a < 3; a++) {
+    const int b0 = (a + 1) % 3, b1 = (a + 2) % 3;
+    const long long nt = (long long)(g.n(b0) + 2 * G + 1) * (g.n(b1) + 2 * G + 1);
+    dim3 grid((unsigned)((nt + 127) / 128), 1, fa.nf);
+    k_fill_axis<<<grid, 128, 0, h->s>>>(h->base, g, fa, a);
+    CKL("k_fill_axis");
+  }
+  return GRMHD_OK;
+}
+
+FillArgs fill_prims() {
+  FillArgs fa{};
+  fa.nf = 5;
+  for (int r = 0; r < 5; r++) { fa.id[r] = F_P + r; fa.stag[r] = 0; fa.kind[r] = 0; }
+  return fa;
+}
+FillArgs fill_vecpot() {
+  FillArgs fa{};
+  fa.nf = 3;
+  const int st[3] = {2 | 4, 1 | 4, 1 | 2};  // A_x on (y,z)-staggered edges, ...
+  for (int d = 0; d < 3; d++) { fa.id[d] = F_Y + 5 + d; fa.stag[d] = st[d]; fa.kind[d] = 1; }
+  return fa;
+}
+
+int set_params(grmhd* h, double cfl, double t_end) {
+  if (cfl != h->cfl_set || h->fixed_dt != h->fixed_set || t_end != h->tend_set) {
+    k_set_params<<<1, 1, 0, h->s>>>(h->dst, cfl, h->fixed_dt, t_end);
+    CKL("k_set_params");
+    h->cfl_set = cfl; h->fixed_set = h->fixed_dt; h->tend_set = t_end;
+  }
+  return GRMHD_OK;
+}
+
+// R13 + R14 + R15 after a change of (U~, A)
+int after_stage(grmhd* h, bool want_speed) {
+  const Geom& g = h->g;
+  int rc = fill_ghosts(h, fill_vecpot());
+  if (rc) return rc;
+  k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+      h->base, g);
+  CKL("k_bfield");
+  k_con2prim<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(
+      h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+  CKL("k_con2prim");
+  return fill_ghosts(h, fill_prims());
+}
+
+int compute_fluxes(grmhd* h) {
+  const Geom& g = h->g;
+  k_flux_face<0><<<grd3(g.nx + 1, g.ny + 2, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
+  CKL("k_flux_face<0>");
+  k_flux_face<1><<<grd3(g.nx + 2, g.ny + 1, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
+  CKL("k_flux_face<1>");
+  k_flux_face<2><<<grd3(g.nx + 2, g.ny + 2, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E);
+  CKL("k_flux_face<2>");
+  return GRMHD_OK;
+}
+
+int one_step(grmhd* h) {
+  const Geom& g = h->g;
+  k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 0);
+  CKL("k_dt");
+  RkStage st[4];
+  int ns = h->o.rk;
+  if (ns == 2) {
+    st[0] = {0, 0, 0, 0}; st[1] = {1, 0.5, 0.5, 0};
+  } else if (ns == 3) {
+    st[0] = {0, 0, 0, 0}; st[1] = {1, 0.75, 0.25, 0}; st[2] = {1, 1.0 / 3.0, 2.0 / 3.0, 0};
+  } else {
+    st[0] = {2, 0, 0, 0}; st[1] = {3, 0, 0, 0.5}; st[2] = {3, 0, 0, 1.0}; st[3] = {4, 0, 0, 0};
+  }
+  for (int s = 0; s < ns; s++) {
+    int rc = compute_fluxes(h);
+    if (rc) return rc;
+    k_update<<<grd3(g.nx + 1, g.ny + 1, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E, h->dst,
+                                                                     st[s]);
+    CKL("k_update");
+    rc = after_stage(h, s == ns - 1);
+    if (rc) return rc;
+  }
+  k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 1);
+  CKL("k_dt");
+  h->steps++;
+  return GRMHD_OK;
+}
+
+// field_from_potential + prim->cons + max speed
+int init_state(grmhd* h) {
+  const Geom& g = h->g;
+  int rc = fill_ghosts(h, fill_vecpot());
+  if (rc) return rc;
+  k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+      h->base, g);
+  CKL("k_bfield");
+  k_prim2con<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(h->base, g, h->E);
+  CKL("k_prim2con");
+  k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 0);
+  CKL("k_reset_state");
+  k_maxspeed<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(h->base, g, h->E, h->dst);
+  CKL("k_maxspeed");
+  return GRMHD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t grmhd_workspace_bytes(int nx, int ny, int nz, int ghosts, const grmhd_opts* opts) {
+  Geom g;
+  if (ghosts != G || !valid_opts(opts) || !make_geom(nx, ny, nz, nullptr, opts, &g)) return 0;
+  const size_t fields = (size_t)nfields_of(opts) * g.NPA * sizeof(double);
+  const size_t stage = (size_t)stage_elems_of(g) * sizeof(double);
+  const size_t mask = (size_t)g.NPA;  // bytes, multiple of 32
+  return fields + stage + mask + 256;
+}
+
+int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3], const grmhd_opts* opts,
+                 void* workspace, size_t workspace_bytes, void* stream, grmhd** out) {
+  if (!out) return GRMHD_EINVAL;
+  *out = nullptr;
+  if (!dx || !workspace || ghosts != G || !valid_opts(opts)) return GRMHD_EINVAL;
+  const int n[3] = {nx, ny, nz};
+  for (int a = 0; a < 3; a++) {
+    if (n[a] < 1 || !(dx[a] > 0)) return GRMHD_EINVAL;
+    if (opts->bc[a] == 1 && n[a] < 2) return GRMHD_EINVAL;
+  }
+  if (((uintptr_t)workspace & 255) != 0) return GRMHD_EINVAL;
+  const size_t need = grmhd_workspace_bytes(nx, ny, nz, ghosts, opts);
+  if (need == 0) return GRMHD_EINVAL;
+  if (workspace_bytes < need) return GRMHD_ENOMEM;
+  grmhd* h = new (std::nothrow) grmhd;
+  if (!h) return GRMHD_ENOMEM;
+  make_geom(nx, ny, nz, dx, opts, &h->g);
+  h->o = *opts;
+  h->E = make_eos(*opts);
+  h->nfields = nfields_of(opts);
+  h->stage_elems = stage_elems_of(h->g);
+  h->base = (double*)workspace;
+  h->stage = h->base + (size_t)h->nfields * h->g.NPA;
+  h->mask = (unsigned char*)(h->stage + h->stage_elems);
+  h->dst = (DevState*)(h->mask + h->g.NPA);
+  h->s = (cudaStream_t)stream;
+  // the whole workspace starts as zeros (ghost cells of U~ stay 0 for the handle's lifetime)
+  cudaError_t e = cudaMemsetAsync(workspace, 0, need, h->s);
+  if (e != cudaSuccess) {
+    delete h;
+    return GRMHD_ECUDA;
+  }
+  *out = h;
+  return GRMHD_OK;
+}
+
+int grmhd_destroy(grmhd* h) {
+  if (!h) return GRMHD_EINVAL;
+  cudaStreamSynchronize(h->s);
+  delete h;
+  return GRMHD_OK;
+}
+
+int grmhd_set_metric(grmhd* h, const double* const field[16]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "set_metric: NULL field array");
+  for (int f = 0; f < 16; f++)
+    if (!field[f]) return fail(h, GRMHD_EINVAL, "set_metric: NULL field");
+  for (int f = 0; f < 16; f++) {
+    int rc = copy_in(h, field[f], F_MET + f, false);
+    if (rc) return rc;
+  }
+  h->have_metric = true;
+  return GRMHD_OK;
+}
+
+int grmhd_set_prims(grmhd* h, const double* const field[8]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "set_prims: NULL field array");
+  if (!h->have_metric) return fail(h, GRMHD_ESTATE, "set_prims before set_metric");
+  for (int r = 0; r < 5; r++)
+    if (!field[r]) return fail(h, GRMHD_EINVAL, "set_prims: NULL hydro field");
+  const bool haveB = field[5] && field[6] && field[7];
+  if (!haveB && (field[5] || field[6] || field[7]))
+    return fail(h, GRMHD_EINVAL, "set_prims: B fields must be all given or all NULL");
+  const Geom& g = h->g;
+  int rc;
+  for (int r = 0; r < 5; r++)
+    if ((rc = copy_in(h, field[r], F_P + r, false))) return rc;
+  if ((rc = fill_ghosts(h, fill_prims()))) return rc;
+  for (int d = 0; d < 3; d++) {
+    if ((rc = zero_field(h, F_Y + 5 + d))) return rc;
+    if ((rc = zero_field(h, F_B0 + d))) return rc;
+  }
+  if (haveB) {
+    // G16: B~0 on faces from the ghost-filled cell-centred input (held in F_BF meanwhile)
+    FillArgs fa{};
+    fa.nf = 3;
+    for (int d = 0; d < 3; d++) {
+      if ((rc = copy_in(h, field[5 + d], F_BF + d, false))) return rc;
+      fa.id[d] = F_BF + d; fa.stag[d] = 0; fa.kind[d] = 0;
+    }
+    if ((rc = fill_ghosts(h, fa))) return rc;
+    for (int d = 0; d < 3; d++) {
+      k_b0_from_centred<<<grd3(g.nx + (d == 0), g.ny + (d == 1), g.nz + (d == 2)), blk3(), 0,
+                          h->s>>>(h->base, g, d);
+      CKL("k_b0_from_centred");
+      fa.id[d] = F_B0 + d; fa.stag[d] = 1 << d; fa.kind[d] = 0;
+    }
+    if ((rc = fill_ghosts(h, fa))) return rc;
+  }
+  h->have_prims = true;
+  h->steps = 0;
+  k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 1);
+  CKL("k_reset_state");
+  return init_state(h);
+}
+
+int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "set_vecpot: NULL field array");
+  if (!h->have_prims) return fail(h, GRMHD_ESTATE, "set_vecpot before set_prims");
+  for (int d = 0; d < 3; d++)
+    if (!field[d]) return fail(h, GRMHD_EINVAL, "set_vecpot: NULL field");
+  for (int d = 0; d < 3; d++) {
+    int rc = copy_in(h, field[d], F_Y + 5 + d, true);
+    if (rc) return rc;
+  }
+  return init_state(h);
+}
+
+int grmhd_set_mask(grmhd* h, const unsigned char* mask) {
+  if (!h) return GRMHD_EINVAL;
+  if (!mask) { h->have_mask = false; return GRMHD_OK; }
+  const Geom& g = h->g;
+  const long long n = (long long)(g.nx + 2 * G) * (g.ny + 2 * G) * (g.nz + 2 * G);
+  const unsigned char* src = mask;
+  if (!is_device_ptr(mask)) {
+    CK(cudaMemcpyAsync(h->stage, mask, (size_t)n, cudaMemcpyDefault, h->s));
+    src = (const unsigned char*)h->stage;
+  }
+  k_repack_mask<<<grd1(n), 256, 0, h->s>>>(src, h->mask, g);
+  CKL("k_repack_mask");
+  h->have_mask = true;
+  return GRMHD_OK;
+}
+
+int grmhd_step(grmhd* h, int n, double cfl) {
+  if (!h) return GRMHD_EINVAL;
+  if (n < 0) return fail(h, GRMHD_EINVAL, "step: n < 0");
+  if (!h->have_metric || !h->have_prims) return fail(h, GRMHD_ESTATE, "step before set_metric/set_prims");
+  int rc = set_params(h, cfl, -1.0);
+  if (rc) return rc;
+  for (int s = 0; s < n; s++)
+    if ((rc = one_step(h))) return rc;
+  return GRMHD_OK;
+}
+
+int grmhd_step_until(grmhd* h, double t_end, double cfl, int* nsteps_done) {
+  if (!h) return GRMHD_EINVAL;
+  if (!h->have_metric || !h->have_prims) return fail(h, GRMHD_ESTATE, "step_until before set_metric/set_prims");
+  if (t_end < 0) return fail(h, GRMHD_EINVAL, "step_until: t_end < 0");
+  int rc = set_params(h, cfl, t_end);
+  if (rc) return rc;
+  int n = 0;
+  for (;;) {
+    DevState st;
+    CK(cudaMemcpyAsync(&st, h->dst, sizeof st, cudaMemcpyDeviceToHost, h->s));
+    CK(cudaStreamSynchronize(h->s));
+    if (st.bad_dt) return fail(h, GRMHD_ENUMERIC, "dt not finite/positive");
+    if (!(t_end - st.t > 1e-12 * std::fmax(1.0, std::fabs(t_end)))) break;
+    if ((rc = one_step(h))) return rc;
+    n++;
+  }
+  if (nsteps_done) *nsteps_done = n;
+  return GRMHD_OK;
+}
+
+int grmhd_get_prims(grmhd* h, double* const field[8]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "get_prims: NULL field array");
+  for (int r = 0; r < 8; r++) {
+    if (!field[r]) return fail(h, GRMHD_EINVAL, "get_prims: NULL field");
+    int rc = copy_out(h, r < 5 ? F_P + r : F_BC + (r - 5), field[r], false, 0);
+    if (rc) return rc;
+  }
+  CK(cudaStreamSynchronize(h->s));
+  return GRMHD_OK;
+}
+
+int grmhd_get_cons(grmhd* h, double* const field[8]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "get_cons: NULL field array");
+  for (int r = 0; r < 8; r++) {
+    if (!field[r]) return fail(h, GRMHD_EINVAL, "get_cons: NULL field");
+    int rc = copy_out(h, r < 5 ? F_Y + r : F_BC + (r - 5), field[r], false, r < 5 ? 1 : 2);
+    if (rc) return rc;
+  }
+  CK(cudaStreamSynchronize(h->s));
+  return GRMHD_OK;
+}
+
+int grmhd_get_vecpot(grmhd* h, double* const field[3]) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "get_vecpot: NULL field array");
+  for (int d = 0; d < 3; d++) {
+    if (!field[d]) return fail(h, GRMHD_EINVAL, "get_vecpot: NULL field");
+    int rc = copy_out(h, F_Y + 5 + d, field[d], true, 0);
+    if (rc) return rc;
+  }
+  CK(cudaStreamSynchronize(h->s));
+  return GRMHD_OK;
+}
+
+int grmhd_set_option(grmhd* h, const char* key, double value) {
+  if (!h || !key) return GRMHD_EINVAL;
+  if (std::strcmp(key, "fixed_dt") == 0) {
+    h->fixed_dt = value;
+    return GRMHD_OK;
+  }
+  return fail(h, GRMHD_EINVAL, "set_option: unknown key");
+}
+
+int grmhd_get_stats(grmhd* h, grmhd_stats* out) {
+  if (!h || !out) return GRMHD_EINVAL;
+  DevState st;
+  CK(cudaMemcpyAsync(&st, h->dst, sizeof st, cudaMemcpyDeviceToHost, h->s));
+  CK(cudaStreamSynchronize(h->s));
+  out->t = st.t; out->dt = st.dt;
+  for (int d = 0; d < 3; d++) {
+    double v;
+    std::memcpy(&v, &st.ms_acc[d], sizeof v);
+    out->maxspeed[d] = v;
+  }
+  out->steps = h->steps;
+  out->c2p_fail = st.c2p_fail; out->p_fix = st.p_fix; out->atmo = st.atmo;
+  out->w_cap = st.w_cap; out->c2p_maxiter = st.c2p_maxiter;
+  if (st.bad_dt) return fail(h, GRMHD_ENUMERIC, "dt not finite/positive");
+  return GRMHD_OK;
+}
+
+long long grmhd_launch_count(const grmhd* h) { return h ? h->launches : 0; }
+
+const char* grmhd_last_error(const grmhd* h) { return h ? h->err : "NULL handle"; }
+
+// ---- stand-alone batches --------------------------------------------------------------
+int grmhd_prim2con_batch(const double* const prim[8], const double* const metric[10],
+                         double* const cons[8], long long n, const grmhd_opts* opts,
+                         void* stream) {
+  if (!prim || !metric || !cons || n < 0 || !valid_opts(opts)) return GRMHD_EINVAL;
+  BatchPtrs bp{};
+  for (int r = 0; r < 8; r++) { bp.prim[r] = prim[r]; bp.cons[r] = cons[r]; }
+  for (int r = 0; r < 10; r++) bp.met[r] = metric[r];
+  for (int r = 0; r < 8; r++) if (!prim[r] || !cons[r]) return GRMHD_EINVAL;
+  for (int r = 0; r < 10; r++) if (!metric[r]) return GRMHD_EINVAL;
+  if (n == 0) return GRMHD_OK;
+  k_prim2con_batch<<<grd1(n), 256, 0, (cudaStream_t)stream>>>(bp, n, make_eos(*opts));
+  return cudaGetLastError() == cudaSuccess ? GRMHD_OK : GRMHD_ECUDA;
+}
+
+int grmhd_con2prim_batch(const double* const cons[8], const double* const metric[10],
+                         double* const prim[5], int* status, int* iters, long long n,
+                         const grmhd_opts* opts, void* stream) {
+  if (!cons || !metric || !prim || !status || !iters || n < 0 || !valid_opts(opts))
+    return GRMHD_EINVAL;
+  BatchPtrs bp{};
+  for (int r = 0; r < 8; r++) { if (!cons[r]) return GRMHD_EINVAL; bp.prim[r] = cons[r]; }
+  for (int r = 0; r < 10; r++) { if (!metric[r]) return GRMHD_EINVAL; bp.met[r] = metric[r]; }
+  for (int r = 0; r < 5; r++) { if (!prim[r]) return GRMHD_EINVAL; bp.cons[r] = prim[r]; }
+  if (n == 0) return GRMHD_OK;
+  k_con2prim_batch<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
+      bp, status, iters, n, make_eos(*opts));
+  return cudaGetLastError() == cudaSuccess ? GRMHD_OK : GRMHD_ECUDA;
+}
+
+int grmhd_dfma_peak(double* out, long long threads, int iters, void* stream) {
+  if (!out || threads < 1 || iters < 1) return GRMHD_EINVAL;
+  k_dfma_peak<<<(unsigned)((threads + 255) / 256), 256, 0, (cudaStream_t)stream>>>(out, threads,
+                                                                                   iters);
+  return cudaGetLastError() == cudaSuccess ? GRMHD_OK : GRMHD_ECUDA;
+}
+
+}  // extern "C"

@@ -1,0 +1,382 @@
+// kernels_aux.cuh -- layout conversion, ghost fill (A1), B from A (A6/R13), con2prim (A2),
+// max-speed reduction (A8), dt.
+#pragma once
+#include "layout.cuh"
+#include "recon_c2p.cuh"
+
+namespace gk {
+
+__device__ __forceinline__ const double* fld(const double* base, const Geom& g, int id) {
+  return base + (size_t)id * g.NPA;
+}
+__device__ __forceinline__ double* fld(double* base, const Geom& g, int id) {
+  return base + (size_t)id * g.NPA;
+}
+
+__device__ __forceinline__ Met load_met(const double* base, const Geom& g, long long c) {
+  Met M;
+  M.a = fld(base, g, F_MET + 0)[c];
+  M.bx = fld(base, g, F_MET + 1)[c]; M.by = fld(base, g, F_MET + 2)[c];
+  M.bz = fld(base, g, F_MET + 3)[c];
+  M.gxx = fld(base, g, F_MET + 4)[c]; M.gxy = fld(base, g, F_MET + 5)[c];
+  M.gxz = fld(base, g, F_MET + 6)[c]; M.gyy = fld(base, g, F_MET + 7)[c];
+  M.gyz = fld(base, g, F_MET + 8)[c]; M.gzz = fld(base, g, F_MET + 9)[c];
+  return M;
+}
+
+__device__ __forceinline__ Prim load_prim(const double* base, const Geom& g, long long c) {
+  Prim P;
+  P.rho = fld(base, g, F_P + 0)[c]; P.vx = fld(base, g, F_P + 1)[c];
+  P.vy = fld(base, g, F_P + 2)[c]; P.vz = fld(base, g, F_P + 3)[c];
+  P.p = fld(base, g, F_P + 4)[c];
+  P.Bx = fld(base, g, F_BC + 0)[c]; P.By = fld(base, g, F_BC + 1)[c];
+  P.Bz = fld(base, g, F_BC + 2)[c];
+  return P;
+}
+
+// ------------------------------------------------------------------ layout conversion
+// external array (ez, ey, ex), x fastest, element (0,0,0) = grid index (-G,-G,-G)
+// <-> internal padded array.  One thread per external element.
+__global__ void k_repack_in(const double* __restrict__ ext, double* __restrict__ dst, Geom g,
+                            int ex, int ey, int ez) {
+  const long long n = (long long)ex * ey * ez;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n;
+       q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % ex), j = (int)((q / ex) % ey), k = (int)(q / ((long long)ex * ey));
+    dst[g.at(i - G, j - G, k - G)] = ext[q];
+  }
+}
+
+// mode 0: plain copy; mode 1: interior cells only, divided by sqrt(gamma) of the cell
+// (get_cons rows D,S_j,tau), ghosts 0; mode 2: interior cells only, ghosts 0.
+__global__ void k_repack_out(const double* __restrict__ src, double* __restrict__ ext,
+                             const double* __restrict__ base, Geom g, int ex, int ey, int ez,
+                             int mode) {
+  const long long n = (long long)ex * ey * ez;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n;
+       q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % ex) - G, j = (int)((q / ex) % ey) - G,
+              k = (int)(q / ((long long)ex * ey)) - G;
+    const long long c = g.at(i, j, k);
+    double v = src[c];
+    if (mode != 0) {
+      const bool in = i >= 0 && i < g.nx && j >= 0 && j < g.ny && k >= 0 && k < g.nz;
+      if (!in) v = 0.0;
+      else if (mode == 1) v = v / sqrt(det_gamma(load_met(base, g, c)));
+    }
+    ext[q] = v;
+  }
+}
+
+__global__ void k_repack_mask(const unsigned char* __restrict__ ext,
+                              unsigned char* __restrict__ dst, Geom g) {
+  const int ex = g.nx + 2 * G, ey = g.ny + 2 * G, ez = g.nz + 2 * G;
+  const long long n = (long long)ex * ey * ez;
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n;
+       q += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(q % ex), j = (int)((q / ex) % ey), k = (int)(q / ((long long)ex * ey));
+    dst[g.at(i - G, j - G, k - G)] = ext[q];
+  }
+}
+
+__global__ void k_fill_zero(double* __restrict__ p, long long n) {
+  for (long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x; q < n;
+       q += (long long)gridDim.x * blockDim.x)
+    p[q] = 0.0;
+}
+
+// ------------------------------------------------------------------------- ghost fill
+// R15 / PAPER.md:350: one pass along axis `a` for up to 8 fields (blockIdx.z = field).
+// The transverse range is the full padded extent on axes already filled (< a) and the
+// valid range on axes still to come (> a), so that edges and corners end up filled after
+// the x, y, z passes.  stag bit b = field staggered along axis b; kind 0 = copy of the
+// nearest valid value (outflow) , 1 = linear extrapolation layer by layer (A_i); periodic
+// axes wrap with period n (staggered index n = image of 0).
+struct FillArgs {
+  int id[8];
+  int stag[8];  // bit mask
+  int kind[8];
+  int nf;
+};
+
+__global__ void k_fill_axis(double* __restrict__ base, Geom g, FillArgs fa, int a) {
+  const int f = blockIdx.z;
+  if (f >= fa.nf) return;
+  double* q = fld(base, g, fa.id[f]);
+  const int st = fa.stag[f], kind = fa.kind[f];
+  const int b0 = (a + 1) % 3, b1 = (a + 2) % 3;
+  const int lo0 = b0 < a ? -G : 0, hi0 = g.n(b0) - 1 + ((st >> b0) & 1) + (b0 < a ? G : 0);
+  const int lo1 = b1 < a ? -G : 0, hi1 = g.n(b1) - 1 + ((st >> b1) & 1) + (b1 < a ? G : 0);
+  const int n0 = hi0 - lo0 + 1, n1 = hi1 - lo1 + 1;
+  // make the x-like axis the fast thread index whenever it is transverse
+  int t0, t1;
+  {
+    const long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (tid >= (long long)n0 * n1) return;
+    if (b0 == 0 || (b1 != 0 && b0 < b1)) { t0 = (int)(tid % n0); t1 = (int)(tid / n0); }
+    else { t1 = (int)(tid % n1); t0 = (int)(tid / n1); }
+  }
+  int I[3];
+  I[b0] = lo0 + t0; I[b1] = lo1 + t1;
+  const int na = g.n(a), sa = (st >> a) & 1;
+  const bool periodic = g.bc[a] == 0;
+  const int hi = na - 1 + sa, ghi = na + G - 1 + sa;
+  const long long sd = g.stride(a);
+  I[a] = 0;
+  const long long c0 = g.at(I[0], I[1], I[2]);  // index of layer 0 along a
+  if (periodic) {
+    for (int gl = -1; gl >= -G; gl--) {
+      const int src = ((gl % na) + na) % na;
+      q[c0 + gl * sd] = q[c0 + src * sd];
+    }
+    for (int gl = na; gl <= ghi; gl++) {
+      const int src = gl % na;
+      q[c0 + gl * sd] = q[c0 + src * sd];
+    }
+  } else if (kind == 0) {
+    const double vlo = q[c0], vhi = q[c0 + hi * sd];
+    for (int gl = -1; gl >= -G; gl--) q[c0 + gl * sd] = vlo;
+    for (int gl = hi + 1; gl <= ghi; gl++) q[c0 + gl * sd] = vhi;
+  } else {
+    double q1 = q[c0], q2 = q[c0 + sd];
+    for (int gl = -1; gl >= -G; gl--) {
+      const double v = 2.0 * q1 - q2;
+      q[c0 + gl * sd] = v;
+      q2 = q1; q1 = v;
+    }
+    q1 = q[c0 + hi * sd]; q2 = q[c0 + (hi - 1) * sd];
+    for (int gl = hi + 1; gl <= ghi; gl++) {
+      const double v = 2.0 * q1 - q2;
+      q[c0 + gl * sd] = v;
+      q2 = q1; q1 = v;
+    }
+  }
+}
+
+// --------------------------------------------------------------------------- B from A
+// R13: B~^i = B~0^i + [ijk] d_j A_k on faces (eq. 24 PAPER.md:149 with
+// epsilon^{ijk} = [ijk]/sqrt(gamma)), then the cell-centre value as the mean
+// of the two faces divided by sqrt(gamma).  One thread per padded index
+// (i,j,k) in [-G, n+G]; a face whose edges do not all exist keeps the static value.
+__device__ __forceinline__ double face_bx(const double* Ay, const double* Az, const double* B0x,
+                                          const Geom& g, long long c) {
+  return B0x[c] + (Az[c + g.sy] - Az[c]) * g.idx[1] - (Ay[c + g.sz] - Ay[c]) * g.idx[2];
+}
+__device__ __forceinline__ double face_by(const double* Ax, const double* Az, const double* B0y,
+                                          const Geom& g, long long c) {
+  return B0y[c] + (Ax[c + g.sz] - Ax[c]) * g.idx[2] - (Az[c + 1] - Az[c]) * g.idx[0];
+}
+__device__ __forceinline__ double face_bz(const double* Ax, const double* Ay, const double* B0z,
+                                          const Geom& g, long long c) {
+  return B0z[c] + (Ay[c + 1] - Ay[c]) * g.idx[0] - (Ax[c + g.sy] - Ax[c]) * g.idx[1];
+}
+
+__global__ void k_bfield(double* __restrict__ base, Geom g) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - G;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y - G;
+  const int k = blockIdx.z - G;
+  if (i > g.nx + G || j > g.ny + G) return;
+  const long long c = g.at(i, j, k);
+  const double* Ax = fld(base, g, F_Y + 5);
+  const double* Ay = fld(base, g, F_Y + 6);
+  const double* Az = fld(base, g, F_Y + 7);
+  const double* B0x = fld(base, g, F_B0 + 0);
+  const double* B0y = fld(base, g, F_B0 + 1);
+  const double* B0z = fld(base, g, F_B0 + 2);
+  const bool ix = i < g.nx + G, jy = j < g.ny + G, kz = k < g.nz + G;
+  const double bx = (jy && kz) ? face_bx(Ay, Az, B0x, g, c) : B0x[c];
+  const double by = (ix && kz) ? face_by(Ax, Az, B0y, g, c) : B0y[c];
+  const double bz = (ix && jy) ? face_bz(Ax, Ay, B0z, g, c) : B0z[c];
+  fld(base, g, F_BF + 0)[c] = bx;
+  fld(base, g, F_BF + 1)[c] = by;
+  fld(base, g, F_BF + 2)[c] = bz;
+  if (ix && jy && kz) {
+    const double isg = 1.0 / sqrt(det_gamma(load_met(base, g, c)));
+    fld(base, g, F_BC + 0)[c] = 0.5 * (bx + face_bx(Ay, Az, B0x, g, c + 1)) * isg;
+    fld(base, g, F_BC + 1)[c] = 0.5 * (by + face_by(Ax, Az, B0y, g, c + g.sy)) * isg;
+    fld(base, g, F_BC + 2)[c] = 0.5 * (bz + face_bz(Ax, Ay, B0z, g, c + g.sz)) * isg;
+  }
+}
+
+// G16: static face field B~0^d = mean over the two cells sharing the face of
+// sqrt(gamma_c) B^d_c, for faces 0..n_d along d and interior transverse indices.
+// Bin = ghost-filled cell-centred input component (temporarily held in F_BF + d).
+__global__ void k_b0_from_centred(double* __restrict__ base, Geom g, int d) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= g.nx + (d == 0) || j >= g.ny + (d == 1) || k >= g.nz + (d == 2)) return;
+  const long long c = g.at(i, j, k), cm = c - g.stride(d);
+  const double* Bin = fld(base, g, F_BF + d);
+  const double sgc = sqrt(det_gamma(load_met(base, g, c)));
+  const double sgm = sqrt(det_gamma(load_met(base, g, cm)));
+  fld(base, g, F_B0 + d)[c] = 0.5 * (sgm * Bin[cm] + sgc * Bin[c]);
+}
+
+// ------------------------------------------------------------------------- reductions
+__device__ __forceinline__ void block_max3_atomic(double m0, double m1, double m2,
+                                                  unsigned long long* acc) {
+  __shared__ double sm[3][32];
+  const int lane = threadIdx.x & 31;
+  const int tid = threadIdx.x + blockDim.x * threadIdx.y;
+  const int warp = tid >> 5;
+  const int nw = (blockDim.x * blockDim.y + 31) >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    m0 = fmax(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+    m1 = fmax(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+    m2 = fmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+  }
+  if ((tid & 31) == 0) { sm[0][warp] = m0; sm[1][warp] = m1; sm[2][warp] = m2; }
+  __syncthreads();
+  if (warp == 0) {
+    m0 = (tid < nw) ? sm[0][tid] : 0.0;
+    m1 = (tid < nw) ? sm[1][tid] : 0.0;
+    m2 = (tid < nw) ? sm[2][tid] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      m0 = fmax(m0, __shfl_xor_sync(0xffffffffu, m0, o));
+      m1 = fmax(m1, __shfl_xor_sync(0xffffffffu, m1, o));
+      m2 = fmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+    }
+    if (tid == 0) {
+      // non-negative doubles order like their bit patterns: the max is exact and
+      // independent of the order of arrival
+      atomicMax(acc + 0, (unsigned long long)__double_as_longlong(m0));
+      atomicMax(acc + 1, (unsigned long long)__double_as_longlong(m1));
+      atomicMax(acc + 2, (unsigned long long)__double_as_longlong(m2));
+    }
+  }
+  (void)lane;
+}
+
+// R16: max(|lambda_-|, |lambda_+|) per direction at a cell centre
+__device__ __forceinline__ void cell_speeds(const Prim& P, const Met& M, const Eos& E,
+                                            double s[3]) {
+  const double idet = 1.0 / det_gamma(M);
+  const Pt pt = point_state(P, M, E);
+  double lm, lp;
+  char_speeds<0>(P, pt, M, inv_gamma_dd<0>(M, idet), E, lm, lp);
+  s[0] = fmax(fabs(lm), fabs(lp));
+  char_speeds<1>(P, pt, M, inv_gamma_dd<1>(M, idet), E, lm, lp);
+  s[1] = fmax(fabs(lm), fabs(lp));
+  char_speeds<2>(P, pt, M, inv_gamma_dd<2>(M, idet), E, lm, lp);
+  s[2] = fmax(fabs(lm), fabs(lp));
+#pragma unroll
+  for (int d = 0; d < 3; d++)
+    if (!(s[d] == s[d])) s[d] = 0.0;  // a NaN never wins the max (same as `s > m`)
+}
+
+// -------------------------------------------------------------------------- con2prim
+// A2 (+A8 when want_speed): interior cells.  Reads D~,S~_j,tau~, B_c, gamma_ij; writes
+// rho,v^i,p and, where a floor/cap acted, the rewritten conserved variables.
+__global__ void __launch_bounds__(128)
+k_con2prim(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
+           DevState* __restrict__ st, int want_speed) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  const bool in = i < g.nx && j < g.ny;
+  double s[3] = {0.0, 0.0, 0.0};
+  int bits = 0, iters = 0;
+  if (in) {
+    const long long c = g.at(i, j, k);
+    const Met M = load_met(base, g, c);
+    const double sg = sqrt(det_gamma(M));
+    const double isg = 1.0 / sg;
+    double U[5], P5[5];
+#pragma unroll
+    for (int r = 0; r < 5; r++) U[r] = fld(base, g, F_Y + r)[c] * isg;  // undensitise, eq. (17)
+    const double Bx = fld(base, g, F_BC + 0)[c], By = fld(base, g, F_BC + 1)[c],
+                 Bz = fld(base, g, F_BC + 2)[c];
+    int rewrite;
+    bits = con2prim(U, Bx, By, Bz, M, E, mask != nullptr && mask[c] != 0, P5, iters, rewrite);
+#pragma unroll
+    for (int r = 0; r < 5; r++) fld(base, g, F_P + r)[c] = P5[r];
+    if (rewrite & 1) fld(base, g, F_Y + 0)[c] = sg * U[0];
+    if (rewrite & 2) {
+#pragma unroll
+      for (int r = 1; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
+    }
+    if (want_speed) {
+      const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
+      cell_speeds(P, M, E, s);
+    }
+  }
+  // counters: integer sums and maxima, order independent
+  const unsigned any = __ballot_sync(0xffffffffu, bits != 0);
+  if (any) {
+    const int nf = __popc(__ballot_sync(0xffffffffu, (bits & 2) != 0));
+    const int np = __popc(__ballot_sync(0xffffffffu, (bits & 4) != 0));
+    const int na = __popc(__ballot_sync(0xffffffffu, (bits & 1) != 0));
+    const int nw = __popc(__ballot_sync(0xffffffffu, (bits & 8) != 0));
+    if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) {
+      if (nf) atomicAdd((unsigned long long*)&st->c2p_fail, (unsigned long long)nf);
+      if (np) atomicAdd((unsigned long long*)&st->p_fix, (unsigned long long)np);
+      if (na) atomicAdd((unsigned long long*)&st->atmo, (unsigned long long)na);
+      if (nw) atomicAdd((unsigned long long*)&st->w_cap, (unsigned long long)nw);
+    }
+  }
+  int mi = iters;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mi = max(mi, __shfl_xor_sync(0xffffffffu, mi, o));
+  if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0 && mi > 0)
+    atomicMax((long long*)&st->c2p_maxiter, (long long)mi);
+  if (want_speed) block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
+}
+
+// stand-alone A8 (used after set_prims / set_vecpot)
+__global__ void __launch_bounds__(128)
+k_maxspeed(const double* __restrict__ base, Geom g, Eos E, DevState* __restrict__ st) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  double s[3] = {0.0, 0.0, 0.0};
+  if (i < g.nx && j < g.ny) {
+    const long long c = g.at(i, j, k);
+    cell_speeds(load_prim(base, g, c), load_met(base, g, c), E, s);
+  }
+  block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
+}
+
+// eqs (20)-(22) on the interior: U~ = sqrt(gamma) U(P, B_c)
+__global__ void k_prim2con(double* __restrict__ base, Geom g, Eos E) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= g.nx || j >= g.ny) return;
+  const long long c = g.at(i, j, k);
+  const Met M = load_met(base, g, c);
+  const double sg = sqrt(det_gamma(M));
+  double U[5];
+  prim2con(load_prim(base, g, c), M, E, U);
+#pragma unroll
+  for (int r = 0; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
+}
+
+// ---------------------------------------------------------------------------------- dt
+// R16 / G22: dt = cfl * min_d dx_d / maxspeed_d (or fixed_dt), clipped to t_end when
+// t_end >= 0.  mode 0: start of a step (compute dt, reset the accumulator);
+// mode 1: end of a step (t += dt).
+__global__ void k_dt(DevState* st, Geom g, int mode) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  if (mode == 1) { st->t += st->dt; return; }
+  double dt;
+  double ms[3];
+  for (int d = 0; d < 3; d++) {
+    ms[d] = __longlong_as_double((long long)st->ms_acc[d]);
+    st->ms_used[d] = ms[d];
+    st->ms_acc[d] = 0ull;
+  }
+  if (st->fixed_dt > 0.0) dt = st->fixed_dt;
+  else {
+    double m = INFINITY;
+    for (int d = 0; d < 3; d++) m = fmin(m, g.dx[d] / ms[d]);
+    dt = st->cfl * m;
+  }
+  if (!(dt > 0.0) || !isfinite(dt)) { st->bad_dt = 1; dt = 0.0; }
+  else if (st->t_end >= 0.0 && dt > st->t_end - st->t) dt = st->t_end - st->t;
+  st->dt = dt;
+}
+
+}  // namespace gk

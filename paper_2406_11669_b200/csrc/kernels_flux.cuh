@@ -1,0 +1,184 @@
+// kernels_flux.cuh -- reconstruction + Riemann flux per direction (A3+A4) and the
+// divergence + source + flux-CT + RK update (A5, A6, A7).
+#pragma once
+#include "kernels_aux.cuh"
+
+namespace gk {
+
+// R4: 4-point Lagrange interpolation to the face between cells c-sd and c
+// (adapted per G3)
+__device__ __forceinline__ double lagrange4(const double* __restrict__ q, long long c,
+                                            long long sd) {
+  return (-q[c - 2 * sd] + 9.0 * q[c - sd] + 9.0 * q[c] - q[c + sd]) * 0.0625;
+}
+
+__device__ __forceinline__ Met face_metric(const double* base, const Geom& g, long long c,
+                                           long long sd) {
+  Met M;
+  M.a = lagrange4(fld(base, g, F_MET + 0), c, sd);
+  M.bx = lagrange4(fld(base, g, F_MET + 1), c, sd);
+  M.by = lagrange4(fld(base, g, F_MET + 2), c, sd);
+  M.bz = lagrange4(fld(base, g, F_MET + 3), c, sd);
+  M.gxx = lagrange4(fld(base, g, F_MET + 4), c, sd);
+  M.gxy = lagrange4(fld(base, g, F_MET + 5), c, sd);
+  M.gxz = lagrange4(fld(base, g, F_MET + 6), c, sd);
+  M.gyy = lagrange4(fld(base, g, F_MET + 7), c, sd);
+  M.gyz = lagrange4(fld(base, g, F_MET + 8), c, sd);
+  M.gzz = lagrange4(fld(base, g, F_MET + 9), c, sd);
+  return M;
+}
+
+// ------------------------------------------------------------------------------ fluxes
+// Generic one-thread-per-face kernel (any block shape).  Faces f = 0..n_D along D, transverse
+// cells with the 1-cell apron flux-CT needs (R10).  Face index = index of its upper cell.
+template <int D>
+__global__ void __launch_bounds__(128)
+k_flux_face(double* __restrict__ base, Geom g, Eos E) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - (D == 0 ? 0 : 1);
+  const int j = blockIdx.y * blockDim.y + threadIdx.y - (D == 1 ? 0 : 1);
+  const int k = blockIdx.z - (D == 2 ? 0 : 1);
+  if (i > g.nx || j > g.ny) return;  // k is in range by construction of the grid
+  const long long c = g.at(i, j, k);
+  const long long sd = D == 0 ? 1 : (D == 1 ? g.sy : g.sz);
+  const Met M = face_metric(base, g, c, sd);
+  const double det = det_gamma(M);
+  const double idet = 1.0 / det;
+  const double sgf = sqrt(det);
+  const double gdd = inv_gamma_dd<D>(M, idet);
+
+  // flattening coefficients of cells f-1 and f from p and v^D (G8c)
+  double fL = 0.0, fR = 0.0;
+  if (E.recon == 1 && E.flatten) {
+    const double* pp = fld(base, g, F_P + 4);
+    const double* vv = fld(base, g, F_P + 1 + D);
+    const double p0 = pp[c - 3 * sd], p1 = pp[c - 2 * sd], p3 = pp[c], p4 = pp[c + sd],
+                 p2 = pp[c - sd], p5 = pp[c + 2 * sd];
+    fL = ppm_flatten(p0, p1, p3, p4, vv[c - 2 * sd], vv[c]);
+    fR = ppm_flatten(p1, p2, p4, p5, vv[c - sd], vv[c + sd]);
+  }
+  double qL[8], qR[8];
+#pragma unroll
+  for (int v = 0; v < 8; v++) {
+    const double* q = v < 5 ? fld(base, g, F_P + v) : fld(base, g, F_BC + (v - 5));
+    double cc[6];
+#pragma unroll
+    for (int s = 0; s < 6; s++) cc[s] = q[c + (s - 3) * sd];
+    recon_pair(E.recon, cc, fL, fR, qL[v], qR[v]);
+  }
+  // G6: the normal field is the single-valued staggered one
+  const double Bn = fld(base, g, F_BF + D)[c] / sgf;
+  qL[5 + D] = Bn; qR[5 + D] = Bn;
+  const Prim PL = {qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6], qL[7]};
+  const Prim PR = {qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6], qR[7]};
+  double out[7];
+  riemann_face<D>(PL, PR, M, sgf, gdd, E, out);
+  const int fid = D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ);
+#pragma unroll
+  for (int r = 0; r < 7; r++) fld(base, g, fid + r)[c] = out[r];
+}
+
+// ------------------------------------------------------------------------------ update
+// RK stage combination (R12 / G15).  mode: 0 first SSP stage (saves Y0), 1 later SSP stage
+// y = a Y0 + b (y + dt k), 2 first RK4 stage, 3 middle RK4 stages y = Y0 + (c dt) k,
+// 4 last RK4 stage y = Y0 + dt/6 (k1 + 2 k2 + 2 k3 + k4).
+struct RkStage {
+  int mode;
+  double a, b, c;
+};
+
+__device__ __forceinline__ void rk_apply(double* __restrict__ base, const Geom& g, int r,
+                                         long long c, double k, double h, const RkStage& s) {
+  double* y = fld(base, g, F_Y + r) + c;
+  double* y0 = fld(base, g, F_Y0 + r) + c;
+  double* ks = fld(base, g, F_KS + r) + c;
+  const double yc = *y;
+  switch (s.mode) {
+    case 0: *y0 = yc; *y = yc + h * k; break;
+    case 1: *y = s.a * (*y0) + s.b * (yc + h * k); break;
+    case 2: *y0 = yc; *ks = k; *y = yc + (0.5 * h) * k; break;
+    case 3: *ks += 2.0 * k; *y = *y0 + (s.c * h) * k; break;
+    default: *y = *y0 + (h / 6.0) * (*ks + k); break;
+  }
+}
+
+__device__ __forceinline__ double d4(const double* __restrict__ q, long long c, long long sd,
+                                     double i12dx) {
+  // 4th-order centred derivative (G12); this operand order gives exactly 0 on constants
+  return (8.0 * (q[c + sd] - q[c - sd]) - (q[c + 2 * sd] - q[c - 2 * sd])) * i12dx;
+}
+
+// One thread per index (i,j,k) in [0,nx]x[0,ny]x[0,nz]: the cell's hydro update (if it is
+// an interior cell) and the three edges attached to it in the lower convention.
+__global__ void __launch_bounds__(128)
+k_update(double* __restrict__ base, Geom g, Eos E, const DevState* __restrict__ st, RkStage rk) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i > g.nx || j > g.ny) return;
+  const long long c = g.at(i, j, k);
+  const double h = st->dt;
+  const long long sy = g.sy, sz = g.sz;
+
+  if (i < g.nx && j < g.ny && k < g.nz) {
+    // R8: L(U~) = -sum_d (F~_{i+1/2} - F~_{i-1/2})/dx_d + alpha sqrt(gamma) S, eq. (17)
+    const Met M = load_met(base, g, c);
+    const Prim P = load_prim(base, g, c);
+    const SrcCoef sc = source_coef(P, M, E);
+    const double asg = M.a * sqrt(det_gamma(M));
+    double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    // S_tau, curvature part: 2 C^{ik} K_ik
+    S[4] = 2.0 * contract(sc.C, fld(base, g, F_MET + 10)[c], fld(base, g, F_MET + 11)[c],
+                          fld(base, g, F_MET + 12)[c], fld(base, g, F_MET + 13)[c],
+                          fld(base, g, F_MET + 14)[c], fld(base, g, F_MET + 15)[c]);
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      const long long sd = a == 0 ? 1 : (a == 1 ? sy : sz);
+      const double w = g.idx[a] * (1.0 / 12.0);
+      const double da = d4(fld(base, g, F_MET + 0), c, sd, w);
+      const double dbx = d4(fld(base, g, F_MET + 1), c, sd, w);
+      const double dby = d4(fld(base, g, F_MET + 2), c, sd, w);
+      const double dbz = d4(fld(base, g, F_MET + 3), c, sd, w);
+      const double cg = contract(sc.C, d4(fld(base, g, F_MET + 4), c, sd, w),
+                                 d4(fld(base, g, F_MET + 5), c, sd, w),
+                                 d4(fld(base, g, F_MET + 6), c, sd, w),
+                                 d4(fld(base, g, F_MET + 7), c, sd, w),
+                                 d4(fld(base, g, F_MET + 8), c, sd, w),
+                                 d4(fld(base, g, F_MET + 9), c, sd, w));
+      S[1 + a] = cg - sc.T00a * da + sc.T0lx * dbx + sc.T0ly * dby + sc.T0lz * dbz;
+      S[4] -= (a == 0 ? sc.ax : (a == 1 ? sc.ay : sc.az)) * da;
+    }
+#pragma unroll
+    for (int r = 0; r < 5; r++) {
+      const double* Fx = fld(base, g, F_FX + r);
+      const double* Fy = fld(base, g, F_FY + r);
+      const double* Fz = fld(base, g, F_FZ + r);
+      double div = (Fx[c + 1] - Fx[c]) * g.idx[0];
+      div += (Fy[c + sy] - Fy[c]) * g.idx[1];
+      div += (Fz[c + sz] - Fz[c]) * g.idx[2];
+      rk_apply(base, g, r, c, -div + asg * S[r], h, rk);
+    }
+  }
+  // R10 (flux-CT, G13/G14) and R11 (d_t A_i = -E_i).  Stored B rows:
+  // FX+5 = F~x(B~y), FX+6 = F~x(B~z); FY+5 = F~y(B~z), FY+6 = F~y(B~x);
+  // FZ+5 = F~z(B~x), FZ+6 = F~z(B~y).
+  const double* FxBy = fld(base, g, F_FX + 5);
+  const double* FxBz = fld(base, g, F_FX + 6);
+  const double* FyBz = fld(base, g, F_FY + 5);
+  const double* FyBx = fld(base, g, F_FY + 6);
+  const double* FzBx = fld(base, g, F_FZ + 5);
+  const double* FzBy = fld(base, g, F_FZ + 6);
+  if (i < g.nx) {  // E_x at (i, j-1/2, k-1/2)
+    const double Ex = 0.25 * (-FyBz[c - sz] - FyBz[c] + FzBy[c - sy] + FzBy[c]);
+    rk_apply(base, g, 5, c, -Ex, h, rk);
+  }
+  if (j < g.ny) {  // E_y at (i-1/2, j, k-1/2)
+    const double Ey = 0.25 * (-FzBx[c - 1] - FzBx[c] + FxBz[c - sz] + FxBz[c]);
+    rk_apply(base, g, 6, c, -Ey, h, rk);
+  }
+  if (k < g.nz) {  // E_z at (i-1/2, j-1/2, k)
+    const double Ez = 0.25 * (-FxBy[c - sy] - FxBy[c] + FyBx[c - 1] + FyBx[c]);
+    rk_apply(base, g, 7, c, -Ez, h, rk);
+  }
+}
+
+}  // namespace gk

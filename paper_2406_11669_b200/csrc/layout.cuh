@@ -1,0 +1,64 @@
+// layout.cuh -- data layout of a handle in HBM.
+//
+// One block of nx*ny*nz cells with G = 3 ghost layers.  Every field, cell
+// centred or staggered, lives in an array of the same padded extent (PZ, PY, PXP), x
+// fastest, structure-of-arrays, fields back to back at a stride of NPA doubles:
+//   PXP = roundup(nx + 8, 4)   x pitch: rows are whole 32-byte sectors; cell i = 0 sits at
+//                              x index X0 = 4 so interior rows start sector aligned
+//   PY  = ny + 7, PZ = nz + 7  (room for the staggered index n + G)
+// Staggered fields use the LOWER convention: index (i,j,k) of A_z is the
+// edge (i-1/2, j-1/2, k), of a d-face field the face i_d - 1/2.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+
+namespace gk {
+
+constexpr int G = 3;
+constexpr int X0 = 4;
+
+struct Geom {
+  int nx, ny, nz;
+  int PXP, PY, PZ;
+  long long sy, sz;  // strides of j and k
+  long long NP;      // PXP*PY*PZ
+  long long NPA;     // field stride (NP rounded up to 32 doubles = 256 B)
+  double dx[3], idx[3];
+  int bc[3];
+
+  __host__ __device__ long long at(int i, int j, int k) const {
+    return (long long)(k + G) * sz + (long long)(j + G) * sy + (i + X0);
+  }
+  __host__ __device__ int n(int a) const { return a == 0 ? nx : (a == 1 ? ny : nz); }
+  __host__ __device__ long long stride(int a) const { return a == 0 ? 1 : (a == 1 ? sy : sz); }
+};
+
+// field ids (units of NPA doubles from the workspace base)
+enum FieldId {
+  F_MET = 0,    // 16: alpha, beta^i, gamma_ij (6), K_ij (6)
+  F_P = 16,     // 5 : rho, v^x, v^y, v^z, p                        cell centres
+  F_BC = 21,    // 3 : Eulerian B^i at cell centres
+  F_BF = 24,    // 3 : densitised B~^d on d-faces (total)
+  F_B0 = 27,    // 3 : static part B~0 (G16)
+  F_Y = 30,     // 8 : evolved D~, S~_j, tau~ (cells) and A_i (edges)
+  F_Y0 = 38,    // 8 : RK register Y^0
+  F_FX = 46,    // 7 : stored x-fluxes: D,S_x,S_y,S_z,tau rows + B^y, B^z rows
+  F_FY = 53,    // 7 : y-fluxes (+ B^z, B^x rows)
+  F_FZ = 60,    // 7 : z-fluxes (+ B^x, B^y rows)
+  F_KS = 67,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
+  F_END_RK23 = 67,
+  F_END_RK4 = 75
+};
+
+// device-resident scalars of a handle
+struct DevState {
+  double t, dt;
+  double cfl, fixed_dt, t_end;       // inputs of the dt kernel (t_end < 0: no clipping)
+  unsigned long long ms_acc[3];      // bit patterns of max |lambda| per direction (A8)
+  double ms_used[3];                 // speeds the last dt was computed from
+  long long c2p_fail, p_fix, atmo, w_cap, c2p_maxiter;
+  int bad_dt;
+  int pad;
+};
+
+}  // namespace gk

@@ -1,0 +1,218 @@
+// phys.cuh -- per-point device arithmetic of the GRMHD substep (fp64, sm_100a).
+//
+// Everything here is a restatement, in register-friendly form, of formulas printed in the
+// AsterX paper (arXiv 2406.11669; PAPER.md) or of the readings listed in DESIGN.md
+// (R-rows = algorithm steps, G-rows = readings where the paper is silent).  No code is
+// shared with oracle/ (the CPU checker); the two are compared by tests/ only.
+//
+// Conventions: prim = (rho, v^x, v^y, v^z, p, B^x, B^y, B^z) with Eulerian v^i, B^i
+// (PAPER.md:98-105); metric = (alpha, beta^i, gamma_ij); cons = undensitised
+// (D, S_j, tau, B^k) of eqs (20)-(22).
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace gk {
+
+struct Met {
+  double a, bx, by, bz, gxx, gxy, gxz, gyy, gyz, gzz;
+};
+
+struct Prim {
+  double rho, vx, vy, vz, p, Bx, By, Bz;
+};
+
+// Constant options of a handle, passed by value to kernels.
+struct Eos {
+  double Gamma;     // ideal-fluid index, eq. (46)
+  double GoGm1;     // Gamma/(Gamma-1):  rho h = rho + GoGm1 p  (h = 1+eps+p/rho)
+  double gm1oG;     // (Gamma-1)/Gamma
+  double rho_atm;
+  double p_atm;     // max(K rho_atm^Gamma_p, p_floor), eqs (47)-(48) PAPER.md:340-342
+  double p_floor;
+  double v2max;     // 1 - 1/w_max^2 (G20)
+  double c2p_tol;
+  int c2p_maxit;
+  int recon;        // 0 minmod, 1 PPM
+  int flatten;
+  int riemann;      // 0 HLLE eq. (29), 1 LxF eq. (30)
+};
+
+__device__ __forceinline__ double sq(double x) { return x * x; }
+
+__device__ __forceinline__ double det_gamma(const Met& M) {
+  return M.gxx * (M.gyy * M.gzz - M.gyz * M.gyz) - M.gxy * (M.gxy * M.gzz - M.gyz * M.gxz) +
+         M.gxz * (M.gxy * M.gyz - M.gyy * M.gxz);
+}
+
+// upper metric gamma^{ij} (6 components), given 1/det
+struct Sym3 {
+  double xx, xy, xz, yy, yz, zz;
+};
+__device__ __forceinline__ Sym3 inv_gamma(const Met& M, double idet) {
+  Sym3 u;
+  u.xx = (M.gyy * M.gzz - M.gyz * M.gyz) * idet;
+  u.xy = (M.gxz * M.gyz - M.gxy * M.gzz) * idet;
+  u.xz = (M.gxy * M.gyz - M.gxz * M.gyy) * idet;
+  u.yy = (M.gxx * M.gzz - M.gxz * M.gxz) * idet;
+  u.yz = (M.gxz * M.gxy - M.gxx * M.gyz) * idet;
+  u.zz = (M.gxx * M.gyy - M.gxy * M.gxy) * idet;
+  return u;
+}
+
+// gamma^{dd} only (R4: the speeds along d need nothing else of the inverse)
+template <int D>
+__device__ __forceinline__ double inv_gamma_dd(const Met& M, double idet) {
+  if (D == 0) return (M.gyy * M.gzz - M.gyz * M.gyz) * idet;
+  if (D == 1) return (M.gxx * M.gzz - M.gxz * M.gxz) * idet;
+  return (M.gxx * M.gyy - M.gxy * M.gxy) * idet;
+}
+
+__device__ __forceinline__ void lower(const Met& M, double x, double y, double z, double& lx,
+                                      double& ly, double& lz) {
+  lx = M.gxx * x + M.gxy * y + M.gxz * z;
+  ly = M.gxy * x + M.gyy * y + M.gyz * z;
+  lz = M.gxz * x + M.gyz * y + M.gzz * z;
+}
+
+// ---------------------------------------------------------------------------------------
+// Point state shared by eqs (13), (20)-(22), (37): PAPER.md:102, 129-133, 266.
+struct Pt {
+  double W, iW, v2, vlx, vly, vlz, ab0, b2, blx, bly, blz, rhoh;
+};
+
+__device__ __forceinline__ Pt point_state(const Prim& P, const Met& M, const Eos& E) {
+  Pt s;
+  double Blx, Bly, Blz;
+  lower(M, P.vx, P.vy, P.vz, s.vlx, s.vly, s.vlz);   // v_i = gamma_ij v^j
+  lower(M, P.Bx, P.By, P.Bz, Blx, Bly, Blz);         // B_i
+  s.v2 = s.vlx * P.vx + s.vly * P.vy + s.vlz * P.vz;
+  const double B2 = Blx * P.Bx + Bly * P.By + Blz * P.Bz;
+  const double Bv = P.Bx * s.vlx + P.By * s.vly + P.Bz * s.vlz;
+  const double iW2 = 1.0 - s.v2;
+  s.W = rsqrt(iW2);                  // W = (1 - v^2)^(-1/2)
+  s.iW = iW2 * s.W;                  // 1/W
+  s.ab0 = s.W * Bv;                  // alpha b^0 = W B^i v_i, eq. (13)
+  s.b2 = (B2 + s.ab0 * s.ab0) * iW2; // b^2 = (B^2 + (alpha b^0)^2)/W^2, eq. (13)
+  s.blx = Blx * s.iW + s.ab0 * s.vlx;  // b_i = B_i/W + alpha b^0 v_i, eq. (37)
+  s.bly = Bly * s.iW + s.ab0 * s.vly;
+  s.blz = Blz * s.iW + s.ab0 * s.vlz;
+  s.rhoh = P.rho + E.GoGm1 * P.p;    // rho h for the ideal fluid, eq. (46)
+  return s;
+}
+
+// R2: eqs (20)-(22); U = (D, S_x, S_y, S_z, tau), undensitised.
+__device__ __forceinline__ void prim2con(const Prim& P, const Met& M, const Eos& E,
+                                         double U[5]) {
+  const Pt s = point_state(P, M, E);
+  const double eW2 = (s.rhoh + s.b2) * s.W * s.W;
+  U[0] = P.rho * s.W;
+  U[1] = eW2 * s.vlx - s.ab0 * s.blx;
+  U[2] = eW2 * s.vly - s.ab0 * s.bly;
+  U[3] = eW2 * s.vlz - s.ab0 * s.blz;
+  U[4] = eW2 - (P.p + 0.5 * s.b2) - s.ab0 * s.ab0 - U[0];
+}
+
+// R6 / G9: fast-magnetosonic bound of the characteristic speeds along direction D.
+// a^2 = c_s^2 + v_A^2 - c_s^2 v_A^2 written over one denominator.
+template <int D>
+__device__ __forceinline__ void char_speeds(const Prim& P, const Pt& s, const Met& M, double gdd,
+                                            const Eos& E, double& lm, double& lp) {
+  const double e = s.rhoh + s.b2;
+  const double Gp = E.Gamma * P.p;
+  const double a2 = (Gp * e + s.b2 * (s.rhoh - Gp)) / (s.rhoh * e);
+  const double vd = D == 0 ? P.vx : (D == 1 ? P.vy : P.vz);
+  const double bd = D == 0 ? M.bx : (D == 1 ? M.by : M.bz);
+  const double den = 1.0 - s.v2 * a2;
+  double rad = a2 * (1.0 - s.v2) * (gdd * den - vd * vd * (1.0 - a2));
+  rad = rad < 0.0 ? 0.0 : rad;
+  const double root = sqrt(rad);
+  const double aoden = M.a / den;
+  const double mid = vd * (1.0 - a2);
+  lm = aoden * (mid - root) - bd;
+  lp = aoden * (mid + root) - bd;
+}
+
+// R5 (last part): floors and velocity cap on a reconstructed face state.
+__device__ __forceinline__ void face_floors(Prim& P, const Met& M, const Eos& E) {
+  if (P.rho < E.rho_atm) P.rho = E.rho_atm;
+  if (P.p < E.p_floor) P.p = E.p_floor;
+  double lx, ly, lz;
+  lower(M, P.vx, P.vy, P.vz, lx, ly, lz);
+  const double v2 = lx * P.vx + ly * P.vy + lz * P.vz;
+  if (v2 > E.v2max) {
+    const double f = sqrt(E.v2max / v2);
+    P.vx *= f; P.vy *= f; P.vz *= f;
+  }
+}
+
+// One side of a face: conserved state U[8], coordinate flux G = alpha F^D of eq. (18)
+// (the alpha is reading G10) and the two speeds.
+// Rows: 0 D, 1-3 S_j, 4 tau, 5-7 B^k.
+template <int D>
+__device__ __forceinline__ void side_state(const Prim& P, const Met& M, double gdd,
+                                           const Eos& E, double U[8], double Gf[8], double& lm,
+                                           double& lp) {
+  const Pt s = point_state(P, M, E);
+  const double eW2 = (s.rhoh + s.b2) * s.W * s.W;
+  const double ptot = P.p + 0.5 * s.b2;
+  U[0] = P.rho * s.W;
+  U[1] = eW2 * s.vlx - s.ab0 * s.blx;
+  U[2] = eW2 * s.vly - s.ab0 * s.bly;
+  U[3] = eW2 * s.vlz - s.ab0 * s.blz;
+  U[4] = eW2 - ptot - s.ab0 * s.ab0 - U[0];
+  U[5] = P.Bx; U[6] = P.By; U[7] = P.Bz;
+  const double vtx = M.a * P.vx - M.bx;  // v~^i = alpha v^i - beta^i
+  const double vty = M.a * P.vy - M.by;
+  const double vtz = M.a * P.vz - M.bz;
+  const double vtd = D == 0 ? vtx : (D == 1 ? vty : vtz);
+  const double vd = D == 0 ? P.vx : (D == 1 ? P.vy : P.vz);
+  const double Bd = D == 0 ? P.Bx : (D == 1 ? P.By : P.Bz);
+  const double aBdW = M.a * Bd * s.iW;   // alpha B^d / W
+  const double ap = M.a * ptot;
+  Gf[0] = U[0] * vtd;
+  Gf[1] = U[1] * vtd - s.blx * aBdW + (D == 0 ? ap : 0.0);
+  Gf[2] = U[2] * vtd - s.bly * aBdW + (D == 1 ? ap : 0.0);
+  Gf[3] = U[3] * vtd - s.blz * aBdW + (D == 2 ? ap : 0.0);
+  Gf[4] = U[4] * vtd + ap * vd - s.ab0 * aBdW;
+  Gf[5] = P.Bx * vtd - Bd * vtx;
+  Gf[6] = P.By * vtd - Bd * vty;
+  Gf[7] = P.Bz * vtd - Bd * vtz;
+  char_speeds<D>(P, s, M, gdd, E, lm, lp);
+}
+
+// R7: HLLE eq. (29) PAPER.md:196 or LxF eq. (30) PAPER.md:203 on the face states PL, PR
+// (floors applied here).  Writes sgf * F^ for the rows that are stored: out[0..4] hydro,
+// out[5], out[6] = the two transverse B rows in cyclic order (D+1, D+2)%3.
+template <int D>
+__device__ __forceinline__ void riemann_face(Prim PL, Prim PR, const Met& M, double sgf,
+                                             double gdd, const Eos& E, double out[7]) {
+  face_floors(PL, M, E);
+  face_floors(PR, M, E);
+  double UL[8], UR[8], GL[8], GR[8], lmL, lpL, lmR, lpR;
+  side_state<D>(PL, M, gdd, E, UL, GL, lmL, lpL);
+  side_state<D>(PR, M, gdd, E, UR, GR, lmR, lpR);
+  const double cmax = fmax(0.0, fmax(lpL, lpR));
+  const double cmin = -fmin(0.0, fmin(lmL, lmR));
+  double F[8];
+  if (E.riemann == 1) {
+    const double cw = fmax(cmax, cmin);
+#pragma unroll
+    for (int r = 0; r < 8; r++) F[r] = 0.5 * (GR[r] + GL[r] - cw * (UR[r] - UL[r]));
+  } else if (cmax + cmin < 1e-300) {
+#pragma unroll
+    for (int r = 0; r < 8; r++) F[r] = 0.5 * (GL[r] + GR[r]);
+  } else {
+    const double inv = 1.0 / (cmax + cmin);
+    const double cc = cmax * cmin;
+#pragma unroll
+    for (int r = 0; r < 8; r++)
+      F[r] = (cmin * GR[r] + cmax * GL[r] - cc * (UR[r] - UL[r])) * inv;
+  }
+#pragma unroll
+  for (int r = 0; r < 5; r++) out[r] = sgf * F[r];
+  out[5] = sgf * F[5 + (D + 1) % 3];
+  out[6] = sgf * F[5 + (D + 2) % 3];
+}
+
+}  // namespace gk

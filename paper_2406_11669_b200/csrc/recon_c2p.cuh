@@ -1,0 +1,248 @@
+// recon_c2p.cuh -- reconstruction (R5/G7/G8), con2prim (R14) and source terms (R9/G11).
+// Device-only restatements of PAPER.md:190-192 (reconstruction), PAPER.md:256-295 +
+// PAPER.md:326 (con2prim + atmosphere) and eq. (19) PAPER.md:125 (sources).
+#pragma once
+#include "phys.cuh"
+
+namespace gk {
+
+// ------------------------------------------------------------------------ reconstruction
+// G7: minmod(a,b) = 0 if a*b <= 0 else sign(a) min(|a|,|b|)
+__device__ __forceinline__ double minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  const double m = fmin(fabs(a), fabs(b));
+  return a > 0.0 ? m : -m;
+}
+
+// G8(a): monotonised central slope of a cell from its two neighbours.
+__device__ __forceinline__ double ppm_slope(double qm1, double q0, double qp1) {
+  const double dp = qp1 - q0, dm = q0 - qm1;
+  if (dp * dm > 0.0) {
+    const double d = 0.5 * (qp1 - qm1);
+    const double lim = fmin(fabs(d), fmin(2.0 * fabs(dp), 2.0 * fabs(dm)));
+    return d > 0.0 ? lim : -lim;
+  }
+  return 0.0;
+}
+
+// G8(c): flattening coefficient of a cell from p_{i-2..i+2} and v^d_{i-1}, v^d_{i+1}.
+__device__ __forceinline__ double ppm_flatten(double pm2, double pm1, double pp1, double pp2,
+                                              double vm1, double vp1) {
+  const double dp1 = pp1 - pm1;
+  const double dp2 = pp2 - pm2;
+  if (fabs(dp1) > 0.33 * fmin(pp1, pm1) && vm1 > vp1) {
+    if (dp2 == 0.0) return 1.0;
+    const double f = 10.0 * (dp1 / dp2 - 0.75);
+    return fmin(1.0, fmax(0.0, f));
+  }
+  return 0.0;
+}
+
+// G8(b): 4th-order interface value between cells (q0 | q1) from the two limited slopes.
+__device__ __forceinline__ double ppm_iface(double q0, double q1, double dm0, double dm1) {
+  return 0.5 * (q0 + q1) - (dm1 - dm0) * (1.0 / 6.0);
+}
+
+// G8(c,d): flatten + monotonise the parabola of one cell; qm = q^-_i, qp = q^+_i.
+__device__ __forceinline__ void ppm_limit(double q0, double f, double& qm, double& qp) {
+  qp = f * q0 + (1.0 - f) * qp;
+  qm = f * q0 + (1.0 - f) * qm;
+  if ((qp - q0) * (q0 - qm) <= 0.0) {
+    qp = q0; qm = q0;
+  } else {
+    const double Dq = qp - qm;
+    const double m = q0 - 0.5 * (qp + qm);
+    const double D26 = Dq * Dq * (1.0 / 6.0);
+    if (Dq * m > D26) qm = 3.0 * q0 - 2.0 * qp;
+    else if (-D26 > Dq * m) qp = 3.0 * q0 - 2.0 * qm;
+  }
+}
+
+// Face states of one variable from the 6 cells c[0..5] = f-3..f+2 around face f:
+// qL from cell f-1, qR from cell f.  fL/fR are the flattening coefficients of those cells.
+__device__ __forceinline__ void recon_pair(int recon, const double c[6], double fL, double fR,
+                                           double& qL, double& qR) {
+  if (recon == 0) {
+    qL = c[2] + 0.5 * minmod(c[2] - c[1], c[3] - c[2]);
+    qR = c[3] - 0.5 * minmod(c[3] - c[2], c[4] - c[3]);
+  } else {
+    const double d1 = ppm_slope(c[0], c[1], c[2]);
+    const double d2 = ppm_slope(c[1], c[2], c[3]);
+    const double d3 = ppm_slope(c[2], c[3], c[4]);
+    const double d4 = ppm_slope(c[3], c[4], c[5]);
+    const double i12 = ppm_iface(c[1], c[2], d1, d2);  // interface f-3/2
+    const double i23 = ppm_iface(c[2], c[3], d2, d3);  // interface f-1/2 (this face)
+    const double i34 = ppm_iface(c[3], c[4], d3, d4);  // interface f+1/2
+    double qm = i12, qp = i23;
+    ppm_limit(c[2], fL, qm, qp);
+    qL = qp;
+    qm = i23; qp = i34;
+    ppm_limit(c[3], fR, qm, qp);
+    qR = qm;
+  }
+}
+
+// ---------------------------------------------------------------------------- con2prim
+// R14: Noble 2-D Newton-Raphson on (z, v^2), eqs (36)-(41) PAPER.md:260-295; atmosphere
+// PAPER.md:326; failure policy G17-G20.  U = undensitised (D,S_j,tau) in/out, B^i, metric.
+// Returns status bits: 1 atmosphere, 2 failed solve, 4 pressure fix, 8 W cap.
+// `rewrite` mask tells which of U changed: bit0 -> D, bit1 -> S_j and tau.
+__device__ __forceinline__ int con2prim(double U[5], double Bx, double By, double Bz,
+                                        const Met& M, const Eos& E, bool masked, double P5[5],
+                                        int& iters, int& rewrite) {
+  iters = 0;
+  rewrite = 0;
+  int bits = 0;
+  const double D = U[0], tau = U[4];
+  bool atmo = masked || !(D > E.rho_atm);
+  if (atmo) bits = 1;
+  double rho = 0, vx = 0, vy = 0, vz = 0, p = 0;
+  if (!atmo) {
+    const double idet = 1.0 / det_gamma(M);
+    const Sym3 gu = inv_gamma(M, idet);
+    const double Sx = U[1], Sy = U[2], Sz = U[3];
+    const double Sux = gu.xx * Sx + gu.xy * Sy + gu.xz * Sz;  // S^i
+    const double Suy = gu.xy * Sx + gu.yy * Sy + gu.yz * Sz;
+    const double Suz = gu.xz * Sx + gu.yz * Sy + gu.zz * Sz;
+    const double S2 = Sux * Sx + Suy * Sy + Suz * Sz;
+    double Blx, Bly, Blz;
+    lower(M, Bx, By, Bz, Blx, Bly, Blz);
+    const double B2 = Blx * Bx + Bly * By + Blz * Bz;
+    const double BS = Bx * Sx + By * Sy + Bz * Sz;
+    const double BS2 = BS * BS;
+    const double g1 = E.gm1oG;
+    double z = tau + D, v2 = 0.0;  // G17: stateless initial guess
+    bool conv = false;
+    for (int it = 1; it <= E.c2p_maxit; it++) {
+      iters = it;
+      const double sw = sqrt(1.0 - v2);  // 1/W
+      const double pz = g1 * (z * (1.0 - v2) - D * sw);
+      const double iz = 1.0 / z;
+      const double iz2 = iz * iz, BS2iz3 = BS2 * iz2 * iz;
+      const double B2z = B2 + z;
+      // eqs (40a), (40b) and their Jacobian
+      const double f1 = v2 * B2z * B2z - BS2 * (B2 + 2.0 * z) * iz2 - S2;
+      const double f2 = tau + D - 0.5 * B2 * (1.0 + v2) + 0.5 * BS2 * iz2 - z + pz;
+      const double J11 = 2.0 * B2z * (v2 + BS2iz3);
+      const double J12 = B2z * B2z;
+      const double J21 = -BS2iz3 - 1.0 + g1 * (1.0 - v2);
+      const double J22 = -0.5 * B2 + g1 * (-z + D / (2.0 * sw));
+      const double idetJ = 1.0 / (J11 * J22 - J12 * J21);
+      const double dz = (f2 * J12 - f1 * J22) * idetJ;
+      const double dv = (f1 * J21 - f2 * J11) * idetJ;
+      const double zn = fabs(z + dz);
+      const double vn = fmin(fmax(v2 + dv, 0.0), 1.0 - 1e-12);  // G18
+      const double err = fabs(dz) / zn + fabs(dv);
+      z = zn; v2 = vn;
+      if (!isfinite(err)) break;
+      if (err < E.c2p_tol) { conv = true; break; }
+    }
+    if (!conv || !isfinite(z) || !isfinite(v2)) {
+      atmo = true; bits = 2;
+    } else {
+      // eqs (41a)-(41d); G19: the 1/gamma of (41d) is 1/Gamma
+      const double iW2 = 1.0 - v2;
+      const double iW = sqrt(iW2);
+      rho = D * iW;
+      const double izB = 1.0 / (z + B2);
+      const double BSz = BS / z;
+      vx = (Sux + BSz * Bx) * izB;
+      vy = (Suy + BSz * By) * izB;
+      vz = (Suz + BSz * Bz) * izB;
+      const double eps = (z * iW2 / rho - 1.0) / E.Gamma;
+      p = (E.Gamma - 1.0) * rho * eps;
+      if (!isfinite(rho) || !isfinite(p) || !isfinite(vx) || !isfinite(vy) || !isfinite(vz) ||
+          rho < E.rho_atm) {
+        atmo = true; bits = 2;
+      } else {
+        if (eps < 0.0 || p < E.p_floor) {  // G20 (ii): pressure fix, keep rho and v
+          p = E.p_floor;
+          bits |= 4;
+        }
+        double lx, ly, lz;
+        lower(M, vx, vy, vz, lx, ly, lz);
+        const double vv = lx * vx + ly * vy + lz * vz;
+        if (vv > E.v2max) {  // R14 (8): Lorentz-factor cap
+          const double f = sqrt(E.v2max / vv);
+          vx *= f; vy *= f; vz *= f;
+          bits |= 8;
+        }
+      }
+    }
+  }
+  if (atmo) {  // rho_atm, polytropic p, v = 0, B kept, cons recomputed
+    rho = E.rho_atm; vx = vy = vz = 0.0; p = E.p_atm;
+  }
+  P5[0] = rho; P5[1] = vx; P5[2] = vy; P5[3] = vz; P5[4] = p;
+  if (bits) {
+    Prim P = {rho, vx, vy, vz, p, Bx, By, Bz};
+    double Un[5];
+    prim2con(P, M, E, Un);
+    if (bits & (1 | 2 | 8)) { U[0] = Un[0]; rewrite |= 1; }  // pressure fix alone keeps D
+    U[1] = Un[1]; U[2] = Un[2]; U[3] = Un[3]; U[4] = Un[4];
+    rewrite |= 2;
+  }
+  return bits;
+}
+
+// ----------------------------------------------------------------------------- sources
+// R9 / G11: S of eq. (19) PAPER.md:125 in its exact 3+1 reduction, split in two parts so
+// that derivatives can be consumed one axis at a time:
+//   S_j   = C^{ik} d_j gamma_ik - T^{00} alpha d_j alpha + T^0_i d_j beta^i
+//   S_tau = 2 C^{ik} K_ik - (T^{00} beta^i + T^{0i}) d_i alpha
+// with C^{ik} = 1/2 (T^{00} beta^i beta^k + T^{0i} beta^k + T^{0k} beta^i + T^{ik}).
+struct SrcCoef {
+  Sym3 C;                 // C^{ik}
+  double T00a;            // T^{00} alpha
+  double T0lx, T0ly, T0lz;  // T^0_i = T^{00} beta_i + T^{0k} gamma_ki
+  double ax, ay, az;      // T^{00} beta^i + T^{0i}
+};
+
+__device__ __forceinline__ SrcCoef source_coef(const Prim& P, const Met& M, const Eos& E) {
+  const Pt s = point_state(P, M, E);
+  const double ia = 1.0 / M.a, ia2 = ia * ia;
+  const double idet = 1.0 / det_gamma(M);
+  const Sym3 gu = inv_gamma(M, idet);
+  // four-velocity and comoving field, eq. (13)
+  const double u0 = s.W * ia;
+  const double ux = s.W * (P.vx - M.bx * ia), uy = s.W * (P.vy - M.by * ia),
+               uz = s.W * (P.vz - M.bz * ia);
+  const double b0 = s.ab0 * ia;
+  const double bx = (P.Bx + s.ab0 * ux) * s.iW, by = (P.By + s.ab0 * uy) * s.iW,
+               bz = (P.Bz + s.ab0 * uz) * s.iW;
+  const double e = s.rhoh + s.b2, pt = P.p + 0.5 * s.b2;
+  // T^{mu nu}, eq. (16), with g^{00} = -1/alpha^2, g^{0i} = beta^i/alpha^2,
+  // g^{ij} = gamma^{ij} - beta^i beta^j/alpha^2
+  const double T00 = e * u0 * u0 - pt * ia2 - b0 * b0;
+  const double T0x = e * u0 * ux + pt * M.bx * ia2 - b0 * bx;
+  const double T0y = e * u0 * uy + pt * M.by * ia2 - b0 * by;
+  const double T0z = e * u0 * uz + pt * M.bz * ia2 - b0 * bz;
+  const double pia2 = pt * ia2;
+  const double Txx = e * ux * ux + pt * gu.xx - pia2 * M.bx * M.bx - bx * bx;
+  const double Txy = e * ux * uy + pt * gu.xy - pia2 * M.bx * M.by - bx * by;
+  const double Txz = e * ux * uz + pt * gu.xz - pia2 * M.bx * M.bz - bx * bz;
+  const double Tyy = e * uy * uy + pt * gu.yy - pia2 * M.by * M.by - by * by;
+  const double Tyz = e * uy * uz + pt * gu.yz - pia2 * M.by * M.bz - by * bz;
+  const double Tzz = e * uz * uz + pt * gu.zz - pia2 * M.bz * M.bz - bz * bz;
+  SrcCoef c;
+  c.ax = T00 * M.bx + T0x; c.ay = T00 * M.by + T0y; c.az = T00 * M.bz + T0z;
+  // C^{ik} = 1/2 (beta^i a^k + T^{0k} beta^i ... ) written symmetrically:
+  // T00 b^i b^k + T0i b^k + T0k b^i = a^i b^k + T0k b^i
+  c.C.xx = 0.5 * (c.ax * M.bx + T0x * M.bx + Txx);
+  c.C.xy = 0.5 * (c.ax * M.by + T0y * M.bx + Txy);
+  c.C.xz = 0.5 * (c.ax * M.bz + T0z * M.bx + Txz);
+  c.C.yy = 0.5 * (c.ay * M.by + T0y * M.by + Tyy);
+  c.C.yz = 0.5 * (c.ay * M.bz + T0z * M.by + Tyz);
+  c.C.zz = 0.5 * (c.az * M.bz + T0z * M.bz + Tzz);
+  c.T00a = T00 * M.a;
+  // T^0_i = gamma_ik (T^{00} beta^k + T^{0k})
+  lower(M, c.ax, c.ay, c.az, c.T0lx, c.T0ly, c.T0lz);
+  return c;
+}
+
+__device__ __forceinline__ double contract(const Sym3& C, double xx, double xy, double xz,
+                                           double yy, double yz, double zz) {
+  return C.xx * xx + C.yy * yy + C.zz * zz + 2.0 * (C.xy * xy + C.xz * xz + C.yz * yz);
+}
+
+}  // namespace gk

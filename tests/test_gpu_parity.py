@@ -1,0 +1,212 @@
+"""GPU-vs-oracle parity (run on the B200 box: pytest -m gpu).  Every call goes through the
+C ABI of libgrmhd.so (paper_2406_11669_b200.binding); expected values come from oracle/.
+
+Tolerances (north_star / DESIGN.md "Parity"): relative 1e-11 per conserved field after one
+step, 1e-9 after 100 steps on smooth data, in the norm max|a-b| / max|b| over interior cells
+(vectors scaled by the vector's largest component).  Integer results (status bits, counters,
+iteration counts) are compared exactly where the decision is not at a rounding threshold.
+"""
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2406_11669_b200 import workloads as wl
+from tests.util import cons_errors, interior, make_gpu, make_ref, to_np
+
+pytestmark = pytest.mark.gpu
+
+TOL1 = 1e-11
+TOL100 = 1e-9
+
+
+def _assert_cons(Ug, Ur, tol, what):
+    errs = cons_errors(Ug, Ur)
+    bad = {k: v for k, v in errs.items() if not (v <= tol)}
+    assert not bad, f"{what}: {bad} (all: {errs})"
+    return errs
+
+
+def _one_step_case(w, nsteps=1, tol=TOL1):
+    r = make_ref(w)
+    g = make_gpu(w)
+    # state right after set_*: conserved variables, primitives incl. ghosts, stats
+    _assert_cons(to_np(g.get_cons()), r.get_cons(), 1e-13, w.name + " init")
+    sg, sr = g.stats(), r.stats()
+    np.testing.assert_allclose(sg["maxspeed"], sr["maxspeed"], rtol=1e-13)
+    r.step(nsteps, w.cfl)
+    g.step(nsteps, w.cfl)
+    errs = _assert_cons(to_np(g.get_cons()), r.get_cons(), tol, w.name)
+    sg, sr = g.stats(), r.stats()
+    assert sg["rc"] == 0 and sr["rc"] == 0
+    assert sg["steps"] == sr["steps"] == nsteps
+    np.testing.assert_allclose(sg["t"], sr["t"], rtol=1e-12)
+    np.testing.assert_allclose(sg["dt"], sr["dt"], rtol=1e-12)
+    np.testing.assert_allclose(sg["maxspeed"], sr["maxspeed"], rtol=1e-10)
+    for k in ("c2p_fail", "atmo", "w_cap"):
+        assert sg[k] == sr[k], (k, sg[k], sr[k])
+    # primitives including the filled ghost zones
+    Pg, Pr = to_np(g.get_prims()), r.get_prims()
+    for f in range(8):
+        s = max(np.abs(Pr[f]).max(), 1e-300) if f in (0, 4) else max(
+            max(np.abs(Pr[q]).max() for q in ((1, 2, 3) if f < 4 else (5, 6, 7))), 1e-300)
+        assert np.abs(Pg[f] - Pr[f]).max() / s <= 100 * tol, (w.name, "prim", f)
+    Ag, Ar = to_np(g.get_vecpot()), r.get_vecpot()
+    amax = max(max(np.abs(a).max() for a in Ar), 1e-300)
+    for d in range(3):
+        assert np.abs(Ag[d] - Ar[d]).max() / amax <= tol, (w.name, "A", d)
+    g.close()
+    return errs
+
+
+# ----------------------------------------------------------------------- point kernels
+def test_prim2con_batch_matches_oracle():
+    import torch
+    from paper_2406_11669_b200 import binding
+    prim, met = wl.c2p_states(4099)
+    o = binding.make_opts(gamma_ad=5.0 / 3.0)
+    cons = binding.prim2con_batch(torch.from_numpy(prim).cuda(), torch.from_numpy(met).cuda(),
+                                  o).cpu().numpy()
+    for q in range(0, prim.shape[1], 7):
+        u = ref.prim2con_pt(prim[:, q], met[:, q], 5.0 / 3.0)
+        np.testing.assert_allclose(cons[:, q], u, rtol=2e-13, atol=1e-13 * np.abs(u).max())
+
+
+def test_con2prim_batch_matches_oracle():
+    """Config 4b: iid states with the config-4 marginals; same decisions, same primitives."""
+    import torch
+    from paper_2406_11669_b200 import binding
+    prim, met = wl.c2p_states(4099)
+    kw = dict(gamma_ad=5.0 / 3.0, rho_atm=1e-10, p_floor=1e-10, w_max=100.0)
+    og, orf = binding.make_opts(**kw), ref.make_opts(**kw)
+    cons = np.stack([ref.prim2con_pt(prim[:, q], met[:, q], 5.0 / 3.0)
+                     for q in range(prim.shape[1])], axis=1)
+    # a few degenerate states: below the atmosphere, zero momentum, zero field
+    cons[0, 0] = 1e-12
+    cons[1:4, 1] = 0.0
+    cons[5:8, 2] = 0.0
+    cons = np.ascontiguousarray(cons)
+    P, st, it = binding.con2prim_batch(torch.from_numpy(cons).cuda(),
+                                       torch.from_numpy(met).cuda(), og)
+    P, st, it = P.cpu().numpy(), st.cpu().numpy(), it.cpu().numpy()
+    nbad_it = 0
+    for q in range(cons.shape[1]):
+        p, u, bits, iters = ref.con2prim_pt(cons[:, q], met[:, q], orf)
+        assert st[q] == bits, (q, st[q], bits)
+        nbad_it += int(it[q] != iters)
+        np.testing.assert_allclose(P[0, q], p[0], rtol=1e-10)
+        np.testing.assert_allclose(P[1:4, q], p[1:4], rtol=0, atol=1e-11)
+        rhoh = p[0] + 2.5 * p[4]
+        assert abs(P[4, q] - p[4]) <= 1e-10 * rhoh
+    # iteration counts may differ by one only where the stop test sits at rounding level
+    assert nbad_it <= 0.01 * cons.shape[1]
+
+
+# ------------------------------------------------------------------ one step, all configs
+def test_config1_balsara_one_step():
+    _one_step_case(wl.balsara1(256, 4, 4))
+
+
+def test_config2_blast_one_step_ragged():
+    _one_step_case(wl.blast(44))          # several 32x4 tiles and a ragged tail
+
+
+def test_config3_kerr_one_step():
+    _one_step_case(wl.kerr_blob(40))      # curved metric, mask, vector potential, outflow
+
+
+def test_config4_c2p_stress_one_step():
+    _one_step_case(wl.c2p_stress(36))     # generic metric incl. K_ij, W up to 10
+
+
+def test_config5_bns_one_step_rk4():
+    _one_step_case(wl.bns_like(32))       # RK4 accumulator path
+
+
+def test_minmod_lxf_rk2_variants():
+    w = wl.c2p_stress(20)
+    for kw in (dict(recon=0, rk=2), dict(riemann=1), dict(ppm_flatten=0, rk=4)):
+        w2 = wl.Workload(**{**w.__dict__, "opts": {**w.opts, **kw}})
+        _one_step_case(w2)
+
+
+def test_tiny_and_degenerate_blocks():
+    """1-cell-thick periodic blocks and the smallest outflow block."""
+    _one_step_case(wl.alfven_wave(16, 1, 1, axis=0), nsteps=3)
+    _one_step_case(wl.alfven_wave(1, 16, 1, axis=1), nsteps=3)
+    _one_step_case(wl.alfven_wave(1, 1, 16, axis=2), nsteps=3)
+    _one_step_case(wl.balsara1(8, 2, 2), nsteps=2)
+
+
+# ------------------------------------------------------------------------- many steps
+def test_alfven_100_steps_smooth():
+    w = wl.alfven_wave(64, 4, 4, axis=0)
+    r, g = make_ref(w), make_gpu(w)
+    r.step(100, w.cfl)
+    g.step(100, w.cfl)
+    _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL100, "alfven 100 steps")
+    np.testing.assert_allclose(g.stats()["t"], r.stats()["t"], rtol=1e-11)
+
+
+def test_bns_100_substeps_smooth():
+    w = wl.bns_like(24)
+    r, g = make_ref(w), make_gpu(w)
+    r.step(25, w.cfl)
+    g.step(25, w.cfl)
+    _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL100, "bns 25 RK4 steps")
+
+
+def test_config1_full_run_to_t04():
+    """Config 1 at full size and full length: same number of steps, same final state."""
+    w = wl.balsara1(256, 4, 4)
+    r, g = make_ref(w), make_gpu(w)
+    nr = r.step_until(w.t_end, w.cfl)
+    ng = g.step_until(w.t_end, w.cfl)
+    assert nr == ng
+    _assert_cons(to_np(g.get_cons()), r.get_cons(), 1e-8, "balsara t=0.4")
+    sg, sr = g.stats(), r.stats()
+    assert sg["c2p_fail"] == sr["c2p_fail"] == 0
+    np.testing.assert_allclose(sg["t"], 0.4, rtol=1e-12)
+
+
+# ----------------------------------------------------------------- boundary behaviour
+def test_error_codes():
+    from paper_2406_11669_b200 import binding
+    w = wl.alfven_wave(8, 1, 1)
+    o = binding.make_opts(**w.opts)
+    s = binding.Solver(w.nx, w.ny, w.nz, w.dx, o)
+    with pytest.raises(binding.GrmhdError) as e:
+        s.set_prims(w.prims)
+    assert e.value.code == binding.ESTATE
+    with pytest.raises(binding.GrmhdError) as e:
+        s.step(1, 0.25)
+    assert e.value.code == binding.ESTATE
+    s.set_metric(w.metric)
+    s.set_prims(w.prims)
+    with pytest.raises(binding.GrmhdError) as e:
+        s.set_option("nonsense", 1.0)
+    assert e.value.code == binding.EINVAL
+    with pytest.raises(binding.GrmhdError):
+        binding.Solver(0, 1, 1, w.dx, o)
+    assert s.launch_count() > 0
+    s.close()
+
+
+def test_host_and_device_inputs_agree():
+    """[dev|host] pointers: pinned host, pageable numpy and device tensors give the same state."""
+    import torch
+    from paper_2406_11669_b200 import binding
+    w = wl.c2p_stress(12)
+    outs = []
+    for mode in ("numpy", "pinned", "device"):
+        conv = {"numpy": lambda a: a,
+                "pinned": lambda a: None if a is None else torch.from_numpy(a).pin_memory(),
+                "device": lambda a: None if a is None else torch.from_numpy(a).cuda()}[mode]
+        s = binding.Solver(w.nx, w.ny, w.nz, w.dx, binding.make_opts(**w.opts))
+        s.set_metric([conv(a) for a in w.metric])
+        s.set_prims([conv(a) for a in w.prims])
+        s.step(1, w.cfl)
+        outs.append(to_np(s.get_cons(host=(mode != "device"))))
+        s.close()
+    for o in outs[1:]:
+        for a, b in zip(o, outs[0]):
+            assert np.array_equal(a, b)

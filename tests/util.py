@@ -43,3 +43,22 @@ def cons_errors(Ua, Ub):
     for r, nm in zip((5, 6, 7), ("Bx", "By", "Bz")):
         out[nm] = rel_field_err(Ua[r], Ub[r], bmax)
     return out
+
+
+def make_gpu(w, **override):
+    """The CUDA library on the same workload (imports torch/CUDA lazily)."""
+    from paper_2406_11669_b200 import binding
+    opts = dict(w.opts)
+    opts.update(override)
+    s = binding.Solver(w.nx, w.ny, w.nz, w.dx, binding.make_opts(**opts))
+    s.set_metric(w.metric)
+    s.set_prims(w.prims)
+    if w.vecpot is not None:
+        s.set_vecpot(w.vecpot)
+    if w.mask is not None:
+        s.set_mask(w.mask)
+    return s
+
+
+def to_np(fields):
+    return [f.cpu().numpy() for f in fields]
