@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- zone-updates/s per RK substep of the GRMHD hot path on B200 (contract: see
+DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--n SIZE]
+                  [--impl reference] [--no-cpu-baseline]
+
+A "step" is one full RK step (all stages: every A1-A8 row of the hot path) of one block.
+N > 1 (torchrun): independent replicas, one block per rank, no data-path collective
+("replicas only"); value = zone-substeps of all ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 GRMHD zone-updates/s per RK substep"
+UNIT = "zone-updates/s"
+# algorithmic bytes per cell and direction of the flux kernel:
+# reads P(5)+B_c(3)+B~^d(1)+alpha,beta,gamma(10) = 19 doubles, writes 7
+FLUX_BYTES_PER_CELL_DIR = 26 * 8
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2,
+                    help="index into BASELINE.json configs (0..4); default 2 = 256^3 Kerr-Schild")
+    ap.add_argument("--n", type=int, default=None, help="override the linear size")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-sample-n", type=int, default=48)
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def traffic_for(workload_name):
+    """dram bytes per flux launch from the committed ncu capture, if one exists for this workload."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(workload_name)
+    return None
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def make_workload(args):
+    from paper_2406_11669_b200 import workloads as wl
+    return wl.make(args.config, args.n)
+
+
+def oracle_throughput(w_small, steps, threads):
+    """zone-substeps/s of the oracle, as it stands, on `threads` host cores."""
+    from oracle import ref
+    ref.set_num_threads(threads)
+    r = ref.RefSolver(w_small.nx, w_small.ny, w_small.nz, w_small.dx,
+                      ref.make_opts(**w_small.opts))
+    r.set_metric(w_small.metric)
+    r.set_prims(w_small.prims)
+    if w_small.vecpot is not None:
+        r.set_vecpot(w_small.vecpot)
+    if w_small.mask is not None:
+        r.set_mask(w_small.mask)
+    t0 = time.perf_counter()
+    r.step(steps, w_small.cfl)
+    dt = time.perf_counter() - t0
+    return w_small.ncells * w_small.stages * steps / dt, dt
+
+
+def sample_workload(args):
+    """The bounded CPU sample: the same generator at a reduced linear size."""
+    from paper_2406_11669_b200 import workloads as wl
+    if args.config == 0:
+        return wl.make(0, None), "full config (256x4x4)"
+    n = args.cpu_sample_n
+    return wl.make(args.config, n), f"same generator at {n}^3"
+
+
+def cpu_baseline(args, target_s=12.0):
+    ws, what = sample_workload(args)
+    cores = os.cpu_count() or 1
+    v1, t1 = oracle_throughput(ws, 1, cores)
+    steps = int(max(1, min(200, target_s / max(t1, 1e-3))))
+    v, t = oracle_throughput(ws, steps, cores)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{what}, {steps} RK{ws.stages} steps, {t:.1f} s wall, OpenMP {cores} threads"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    ws, what = sample_workload(args)
+    wfull = None
+    cores = os.cpu_count() or 1
+    for _ in range(max(args.warmup, 0)):
+        oracle_throughput(ws, 1, cores)
+    t0 = time.perf_counter()
+    tot = 0.0
+    for _ in range(args.steps):
+        _, dt = oracle_throughput(ws, 1, cores)
+        tot += dt
+    wall = time.perf_counter() - t0
+    value = ws.ncells * ws.stages * args.steps / tot
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": config_name(args), "sample": what, "stages": ws.stages,
+                       "cells_per_step": ws.ncells},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{what}; each step = one RK{ws.stages} step of the "
+                                       f"oracle, OpenMP {cores} threads; wall {wall:.1f} s"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def config_name(args):
+    names = ["config1_balsara1_256x4x4", "config2_blast_128", "config3_kerrschild_256",
+             "config4_c2p_stress_256", "config5_bns_512"]
+    if args.n is None:
+        return names[args.config]
+    return names[args.config].rsplit("_", 1)[0] + "_%d" % args.n
+
+
+ALG_BYTES = {  # algorithmic bytes per interior cell and launch
+    "flux_x": FLUX_BYTES_PER_CELL_DIR, "flux_y": FLUX_BYTES_PER_CELL_DIR,
+    "flux_z": FLUX_BYTES_PER_CELL_DIR,
+    "update": (49 + 5 + 12 + 3) * 8,      # hydro update 49 r + 5 w, EMF/A update 12 r + 3 w
+    "bfield": (3 + 3 + 6 + 6) * 8,        # A (3) + B~0 (3) + gamma (6) read, B~ (3) + B_c (3) written
+    "con2prim": (5 + 3 + 6 + 5) * 8,      # U~ (5) + B_c (3) + gamma (6) read, P (5) written
+}
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2406_11669_b200 import binding
+
+    w = make_workload(args)
+    opts = binding.make_opts(**w.opts)
+    dev = f"cuda:{local}"
+    s = binding.Solver(w.nx, w.ny, w.nz, w.dx, opts, device=dev)
+    pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
+    h_prims = [pin(a) for a in w.prims]
+    h_vec = None if w.vecpot is None else [pin(a) for a in w.vecpot]
+    s.set_metric(w.metric)
+    if w.mask is not None:
+        s.set_mask(w.mask)
+
+    def reset():
+        s.set_prims(h_prims)
+        if h_vec is not None:
+            s.set_vecpot(h_vec)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput -------------------------------------------------
+    reset()
+    for _ in range(args.warmup):
+        s.step(1, w.cfl)
+    s.set_option("kernel_timing", 1)
+    stream = s.stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = s.launch_count()
+    e0.record(stream)
+    s.step(args.steps, w.cfl)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - l0
+    kt = s.kernel_times()
+    s.set_option("kernel_timing", 0)
+    st = s.stats()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    zone_sub = w.ncells * w.stages * args.steps
+    value = world * zone_sub / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers --------------------------------
+    k_e2e = max(1, min(args.steps, 5))
+    out_host = [torch.empty(s.cc_shape, dtype=torch.float64).pin_memory() for _ in range(8)]
+    reset(); s.step(1, w.cfl); s.get_cons(out=out_host)   # warm-up of the e2e path
+    barrier()
+    t0 = time.perf_counter()
+    e0.record(stream)
+    for _ in range(k_e2e):
+        reset()
+        s.step(1, w.cfl)
+        s.get_cons(out=out_host)
+    e1.record(stream)
+    barrier()
+    wall_e2e = time.perf_counter() - t0
+    ms_e2e = max(e0.elapsed_time(e1), 0.0)
+    if world > 1:
+        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    h2d = sum(a.numel() * 8 for a in h_prims if a is not None) + \
+        (sum(a.numel() * 8 for a in h_vec) if h_vec else 0)
+    d2h = sum(a.numel() * 8 for a in out_host)
+    e2e = {"value": world * w.ncells * w.stages * k_e2e / (ms_e2e * 1e-3), "unit": UNIT,
+           "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": k_e2e,
+           "ms_per_step": ms_e2e / k_e2e,
+           "call": "set_prims[+set_vecpot](pinned host) -> step(1) -> get_cons(pinned host)"}
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return
+
+    # ---- roofline of the dominant kernel --------------------------------------------------
+    peak, peak_src = peaks()
+    kernels = {}
+    tot_k = sum(v[0] for v in kt.values()) or 1.0
+    for k, (kms, cnt) in kt.items():
+        if cnt == 0:
+            continue
+        avg = kms / cnt
+        ent = {"ms_avg": avg, "launches": cnt, "share": kms / tot_k}
+        if k in ALG_BYTES:
+            ent["alg_GBps"] = ALG_BYTES[k] * w.ncells / (avg * 1e-3) / 1e9
+        kernels[k] = ent
+    flux_ms = sum(kt[k][0] for k in ("flux_x", "flux_y", "flux_z"))
+    flux_n = sum(kt[k][1] for k in ("flux_x", "flux_y", "flux_z")) or 1
+    flux_avg = flux_ms / flux_n
+    achieved = FLUX_BYTES_PER_CELL_DIR * w.ncells / (flux_avg * 1e-3) / 1e9
+    roofline = {"kernel": "flux (reconstruct + Riemann, average of x/y/z launches)",
+                "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic_for(w.name),
+                "alg_bytes_per_launch": FLUX_BYTES_PER_CELL_DIR * w.ncells,
+                "ms_per_launch": flux_avg, "share_of_step": flux_ms / tot_k,
+                "peak_source": peak_src,
+                "step_decomposed_frac": (1400.0 * zone_sub / (ms * 1e-3) / 1e9) / peak,
+                "step_floor_frac": (344.0 * zone_sub / (ms * 1e-3) / 1e9) / peak}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "cells": [w.nx, w.ny, w.nz], "ghosts": 3,
+                       "stages_per_step": w.stages, "recon": "ppm" if w.opts["recon"] else "minmod",
+                       "riemann": "hlle", "cfl": w.cfl, "parallelism": "replicas" if world > 1 else "1gpu",
+                       "l2": "inputs larger than L2 (every kernel streams > 126 MB)"
+                             if w.ncells >= 128 ** 3 else "working set fits L2 (latency-bound config)",
+                       "us_per_substep": 1e3 * ms / (args.steps * w.stages)},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "kernels": kernels,
+            "stats": {k: st[k] for k in ("t", "dt", "c2p_fail", "p_fix", "atmo", "w_cap",
+                                         "c2p_maxiter")}}
+    if world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args)
+    print(json.dumps(line))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

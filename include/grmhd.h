@@ -135,12 +135,23 @@ int grmhd_get_prims(grmhd* h, double* const field[8]);
 int grmhd_get_cons(grmhd* h, double* const field[8]);
 int grmhd_get_vecpot(grmhd* h, double* const field[3]);
 
-/* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off).
- * Unknown key -> EINVAL. */
+/* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off);
+ * "kernel_timing" (1: bracket every kernel group of the step with CUDA events on the
+ * handle's stream and accumulate device times, see grmhd_get_kernel_times; 0 = off;
+ * setting it clears the accumulators).  Unknown key -> EINVAL. */
 int grmhd_set_option(grmhd* h, const char* key, double value);
 
 /* Synchronises and copies the counters.  Returns ENUMERIC if any dt was not finite/positive. */
 int grmhd_get_stats(grmhd* h, grmhd_stats* out);
+
+/* Device time per kernel group since "kernel_timing" was switched on (measurement aid for
+ * the roofline report; synchronises).  Groups: 0 flux-x, 1 flux-y, 2 flux-z (A3+A4),
+ * 3 divergence+sources+flux-CT+RK update (A5-A7), 4 A_i ghost fill + B from A (A1,A6),
+ * 5 con2prim (A2, +A8 on the last stage), 6 primitive ghost fill (A1), 7 dt scalars.
+ * ms[q] = summed milliseconds, launches[q] = number of timed brackets. */
+#define GRMHD_NKGROUPS 8
+int grmhd_get_kernel_times(grmhd* h, double ms[GRMHD_NKGROUPS],
+                           long long launches[GRMHD_NKGROUPS]);
 
 /* Number of kernels this handle has launched so far (host-side counter). */
 long long grmhd_launch_count(const grmhd* h);

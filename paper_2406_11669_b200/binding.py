@@ -22,7 +22,7 @@ _ERRNAME = {EINVAL: "GRMHD_EINVAL", ENOMEM: "GRMHD_ENOMEM", ESTATE: "GRMHD_ESTAT
 EXPORTS = ["grmhd_workspace_bytes", "grmhd_create", "grmhd_destroy", "grmhd_set_metric",
            "grmhd_set_prims", "grmhd_set_vecpot", "grmhd_set_mask", "grmhd_step",
            "grmhd_step_until", "grmhd_get_prims", "grmhd_get_cons", "grmhd_get_vecpot",
-           "grmhd_set_option", "grmhd_get_stats", "grmhd_launch_count", "grmhd_last_error",
+           "grmhd_set_option", "grmhd_get_stats", "grmhd_get_kernel_times", "grmhd_launch_count", "grmhd_last_error",
            "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_dfma_peak"]
 
 
@@ -83,6 +83,8 @@ def lib():
         L.grmhd_step_until.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(C.c_int)]
         L.grmhd_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_double]
         L.grmhd_get_stats.argtypes = [C.c_void_p, C.POINTER(GrmhdStats)]
+        L.grmhd_get_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double),
+                                             C.POINTER(C.c_longlong)]
         L.grmhd_launch_count.argtypes = [C.c_void_p]
         L.grmhd_launch_count.restype = C.c_longlong
         L.grmhd_last_error.argtypes = [C.c_void_p]
@@ -243,6 +245,16 @@ class Solver:
         d["maxspeed"] = [s.maxspeed[i] for i in range(3)]
         d["rc"] = rc
         return d
+
+    KERNEL_GROUPS = ("flux_x", "flux_y", "flux_z", "update", "bfield", "con2prim", "ghost_prims",
+                     "dt")
+
+    def kernel_times(self) -> dict:
+        """{group: (summed ms, brackets)} since set_option("kernel_timing", 1)."""
+        ms = (C.c_double * 8)()
+        cnt = (C.c_longlong * 8)()
+        self._chk(lib().grmhd_get_kernel_times(self.h, ms, cnt), "grmhd_get_kernel_times")
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_GROUPS)}
 
     def launch_count(self) -> int:
         return int(lib().grmhd_launch_count(self.h))

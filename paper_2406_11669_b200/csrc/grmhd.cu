@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "kernels_flux.cuh"
 #include "kernels_batch.cuh"
@@ -30,6 +31,13 @@ struct grmhd {
   long long steps = 0;
   long long launches = 0;
   char err[256] = {0};
+  // optional per-kernel-group timing ("kernel_timing" option): CUDA events on the stream
+  bool ktime = false;
+  std::vector<cudaEvent_t> ev;     // pool, used pairwise
+  std::vector<int> ev_grp;         // group of each recorded pair
+  size_t ev_used = 0;
+  double kms[GRMHD_NKGROUPS] = {0};
+  long long kcnt[GRMHD_NKGROUPS] = {0};
 };
 
 namespace {
@@ -55,6 +63,49 @@ int cuda_fail(grmhd* h, cudaError_t e, const char* where) {
     h->launches++;                                                   \
     cudaError_t e_ = cudaGetLastError();                             \
     if (e_ != cudaSuccess) return cuda_fail(h, e_, name);            \
+  } while (0)
+
+// ---- kernel-group timing -------------------------------------------------------------
+enum { KG_FLUX_X = 0, KG_FLUX_Y, KG_FLUX_Z, KG_UPDATE, KG_BFIELD, KG_C2P, KG_GHOST, KG_MISC };
+
+int kt_flush(grmhd* h) {
+  if (h->ev_used == 0) return GRMHD_OK;
+  CK(cudaStreamSynchronize(h->s));
+  for (size_t q = 0; q < h->ev_used; q += 2) {
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, h->ev[q], h->ev[q + 1]));
+    h->kms[h->ev_grp[q / 2]] += ms;
+    h->kcnt[h->ev_grp[q / 2]]++;
+  }
+  h->ev_used = 0;
+  return GRMHD_OK;
+}
+
+int kt_begin(grmhd* h, int grp) {
+  if (!h->ktime) return GRMHD_OK;
+  if (h->ev_used + 2 > h->ev.size()) {
+    int rc = kt_flush(h);
+    if (rc) return rc;
+  }
+  h->ev_grp[h->ev_used / 2] = grp;
+  CK(cudaEventRecord(h->ev[h->ev_used], h->s));
+  return GRMHD_OK;
+}
+
+int kt_end(grmhd* h) {
+  if (!h->ktime) return GRMHD_OK;
+  CK(cudaEventRecord(h->ev[h->ev_used + 1], h->s));
+  h->ev_used += 2;
+  return GRMHD_OK;
+}
+
+#define KT(grp, ...)                               \
+  do {                                             \
+    int rc_ = kt_begin(h, grp);                    \
+    if (rc_) return rc_;                           \
+    __VA_ARGS__;                                   \
+    rc_ = kt_end(h);                               \
+    if (rc_) return rc_;                           \
   } while (0)
 
 bool valid_opts(const grmhd_opts* o) {
@@ -197,32 +248,49 @@ int set_params(grmhd* h, double cfl, double t_end) {
 // R13 + R14 + R15 after a change of (U~, A)
 int after_stage(grmhd* h, bool want_speed) {
   const Geom& g = h->g;
-  int rc = fill_ghosts(h, fill_vecpot());
-  if (rc) return rc;
-  k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
-      h->base, g);
-  CKL("k_bfield");
-  k_con2prim<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(
-      h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
-  CKL("k_con2prim");
-  return fill_ghosts(h, fill_prims());
+  int rc;
+  KT(KG_BFIELD, {
+    rc = fill_ghosts(h, fill_vecpot());
+    if (rc) return rc;
+    k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+        h->base, g);
+    CKL("k_bfield");
+  });
+  KT(KG_C2P, {
+    k_con2prim<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(
+        h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+    CKL("k_con2prim");
+  });
+  KT(KG_GHOST, {
+    rc = fill_ghosts(h, fill_prims());
+    if (rc) return rc;
+  });
+  return GRMHD_OK;
 }
 
 int compute_fluxes(grmhd* h) {
   const Geom& g = h->g;
-  k_flux_face<0><<<grd3(g.nx + 1, g.ny + 2, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
-  CKL("k_flux_face<0>");
-  k_flux_face<1><<<grd3(g.nx + 2, g.ny + 1, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
-  CKL("k_flux_face<1>");
-  k_flux_face<2><<<grd3(g.nx + 2, g.ny + 2, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E);
-  CKL("k_flux_face<2>");
+  KT(KG_FLUX_X, {
+    k_flux_face<0><<<grd3(g.nx + 1, g.ny + 2, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
+    CKL("k_flux_face<0>");
+  });
+  KT(KG_FLUX_Y, {
+    k_flux_face<1><<<grd3(g.nx + 2, g.ny + 1, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
+    CKL("k_flux_face<1>");
+  });
+  KT(KG_FLUX_Z, {
+    k_flux_face<2><<<grd3(g.nx + 2, g.ny + 2, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E);
+    CKL("k_flux_face<2>");
+  });
   return GRMHD_OK;
 }
 
 int one_step(grmhd* h) {
   const Geom& g = h->g;
-  k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 0);
-  CKL("k_dt");
+  KT(KG_MISC, {
+    k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 0);
+    CKL("k_dt");
+  });
   RkStage st[4];
   int ns = h->o.rk;
   if (ns == 2) {
@@ -235,14 +303,18 @@ int one_step(grmhd* h) {
   for (int s = 0; s < ns; s++) {
     int rc = compute_fluxes(h);
     if (rc) return rc;
-    k_update<<<grd3(g.nx + 1, g.ny + 1, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E, h->dst,
-                                                                     st[s]);
-    CKL("k_update");
+    KT(KG_UPDATE, {
+      k_update<<<grd3(g.nx + 1, g.ny + 1, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E,
+                                                                       h->dst, st[s]);
+      CKL("k_update");
+    });
     rc = after_stage(h, s == ns - 1);
     if (rc) return rc;
   }
-  k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 1);
-  CKL("k_dt");
+  KT(KG_MISC, {
+    k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 1);
+    CKL("k_dt");
+  });
   h->steps++;
   return GRMHD_OK;
 }
@@ -316,6 +388,7 @@ int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3], const g
 int grmhd_destroy(grmhd* h) {
   if (!h) return GRMHD_EINVAL;
   cudaStreamSynchronize(h->s);
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   delete h;
   return GRMHD_OK;
 }
@@ -477,6 +550,18 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
     h->fixed_dt = value;
     return GRMHD_OK;
   }
+  if (std::strcmp(key, "kernel_timing") == 0) {
+    int rc = kt_flush(h);
+    if (rc) return rc;
+    h->ktime = value != 0.0;
+    for (int q = 0; q < GRMHD_NKGROUPS; q++) { h->kms[q] = 0.0; h->kcnt[q] = 0; }
+    if (h->ktime && h->ev.empty()) {
+      h->ev.resize(2048);
+      h->ev_grp.resize(1024);
+      for (auto& e : h->ev) CK(cudaEventCreate(&e));
+    }
+    return GRMHD_OK;
+  }
   return fail(h, GRMHD_EINVAL, "set_option: unknown key");
 }
 
@@ -495,6 +580,15 @@ int grmhd_get_stats(grmhd* h, grmhd_stats* out) {
   out->c2p_fail = st.c2p_fail; out->p_fix = st.p_fix; out->atmo = st.atmo;
   out->w_cap = st.w_cap; out->c2p_maxiter = st.c2p_maxiter;
   if (st.bad_dt) return fail(h, GRMHD_ENUMERIC, "dt not finite/positive");
+  return GRMHD_OK;
+}
+
+int grmhd_get_kernel_times(grmhd* h, double ms[GRMHD_NKGROUPS],
+                           long long launches[GRMHD_NKGROUPS]) {
+  if (!h || !ms || !launches) return GRMHD_EINVAL;
+  int rc = kt_flush(h);
+  if (rc) return rc;
+  for (int q = 0; q < GRMHD_NKGROUPS; q++) { ms[q] = h->kms[q]; launches[q] = h->kcnt[q]; }
   return GRMHD_OK;
 }
 

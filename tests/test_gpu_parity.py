@@ -19,8 +19,25 @@ TOL1 = 1e-11
 TOL100 = 1e-9
 
 
+REPORT = []
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _dump_report():
+    """Write the measured parity errors where the GPU run leaves its artefacts."""
+    yield
+    import json
+    import os
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "parity_errors.json"), "w") as f:
+        json.dump(REPORT, f, indent=1)
+
+
 def _assert_cons(Ug, Ur, tol, what):
     errs = cons_errors(Ug, Ur)
+    REPORT.append({"case": what, "tol": tol, "max": float(max(errs.values())),
+                   "errs": {k: float(v) for k, v in errs.items()}})
     bad = {k: v for k, v in errs.items() if not (v <= tol)}
     assert not bad, f"{what}: {bad} (all: {errs})"
     return errs
@@ -123,9 +140,13 @@ def test_config5_bns_one_step_rk4():
 
 
 def test_minmod_lxf_rk2_variants():
-    w = wl.c2p_stress(20)
-    for kw in (dict(recon=0, rk=2), dict(riemann=1), dict(ppm_flatten=0, rk=4)):
-        w2 = wl.Workload(**{**w.__dict__, "opts": {**w.opts, **kw}})
+    for base, kw in ((wl.c2p_stress(20), dict(recon=0, rk=2)),
+                     (wl.c2p_stress(20), dict(riemann=1)),
+                     (wl.blast(20), dict(ppm_flatten=0, rk=4)),
+                     (wl.kerr_blob(20), dict(recon=0, rk=4, riemann=1))):
+        w = base
+        w2 = wl.Workload(**{**w.__dict__, "opts": {**w.opts, **kw},
+                            "name": w.name + "_" + "_".join(f"{k}{v}" for k, v in kw.items())})
         _one_step_case(w2)
 
 
