@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "kernels_flux.cuh"
+#include "flux_march.cuh"
 #include "kernels_batch.cuh"
 
 using namespace gk;
@@ -30,6 +31,7 @@ struct grmhd {
   double cfl_set = -1.0, fixed_dt = 0.0, fixed_set = -1.0, tend_set = -2.0;
   long long steps = 0;
   long long launches = 0;
+  int fm_conc[9] = {0};  // resident blocks of each flux-kernel instantiation (0 = not queried)
   char err[256] = {0};
   // optional per-kernel-group timing ("kernel_timing" option): CUDA events on the stream
   bool ktime = false;
@@ -268,20 +270,58 @@ int after_stage(grmhd* h, bool want_speed) {
   return GRMHD_OK;
 }
 
-int compute_fluxes(grmhd* h) {
+// ---- marching flux kernel launch (flux_march.cuh) ----------------------------------------
+constexpr int FM_TC = 4;
+
+template <int D, int RECON>
+int launch_flux(grmhd* h) {
   const Geom& g = h->g;
-  KT(KG_FLUX_X, {
-    k_flux_face<0><<<grd3(g.nx + 1, g.ny + 2, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
-    CKL("k_flux_face<0>");
-  });
-  KT(KG_FLUX_Y, {
-    k_flux_face<1><<<grd3(g.nx + 2, g.ny + 1, g.nz + 2), blk3(), 0, h->s>>>(h->base, g, h->E);
-    CKL("k_flux_face<1>");
-  });
-  KT(KG_FLUX_Z, {
-    k_flux_face<2><<<grd3(g.nx + 2, g.ny + 2, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E);
-    CKL("k_flux_face<2>");
-  });
+  auto kern = k_flux_march<D, RECON, FM_TC>;
+  const int smem = (int)sizeof(FluxSmem<D, FM_TC>);
+  const int cfg = D * 3 + RECON;
+  if (h->fm_conc[cfg] == 0) {  // first use: opt in to the shared memory, query residency
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int nb = 0, dev = 0, nsm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, FM_THREADS, smem));
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    h->fm_conc[cfg] = nb * nsm > 0 ? nb * nsm : 1;
+  }
+  const int nfaces = g.n(D) + 1;
+  const int ngroups = (fm_npencils(g, D) + 31) / 32;
+  // segments along D: fill whole waves of resident blocks; a segment costs ~2 extra cells
+  int best = 1;
+  double best_cost = 1e300;
+  for (int ns = 1; ns <= 64; ns++) {
+    const int sl = ((nfaces + ns - 1) / ns + FM_TC - 1) / FM_TC * FM_TC;
+    if (ns > 1 && sl < 16) break;
+    const int nseg = (nfaces + sl - 1) / sl;
+    const long long nblk = (long long)nseg * ngroups;
+    const long long waves = (nblk + h->fm_conc[cfg] - 1) / h->fm_conc[cfg];
+    const double cost = (double)waves * (sl + 2);
+    if (cost < best_cost * 0.97) { best_cost = cost; best = ns; }
+  }
+  const int seglen = ((nfaces + best - 1) / best + FM_TC - 1) / FM_TC * FM_TC;
+  const int nseg = (nfaces + seglen - 1) / seglen;
+  kern<<<dim3(ngroups, nseg), FM_THREADS, smem, h->s>>>(h->base, g, h->E, seglen);
+  return GRMHD_OK;
+}
+
+template <int D>
+int launch_flux_d(grmhd* h) {
+  const int recon = h->o.recon == 0 ? 0 : (h->o.ppm_flatten ? 2 : 1);
+  int rc = recon == 0 ? launch_flux<D, 0>(h) : (recon == 1 ? launch_flux<D, 1>(h)
+                                                            : launch_flux<D, 2>(h));
+  if (rc) return rc;
+  CKL("k_flux_march");
+  return GRMHD_OK;
+}
+
+int compute_fluxes(grmhd* h) {
+  int rc;
+  KT(KG_FLUX_X, { if ((rc = launch_flux_d<0>(h))) return rc; });
+  KT(KG_FLUX_Y, { if ((rc = launch_flux_d<1>(h))) return rc; });
+  KT(KG_FLUX_Z, { if ((rc = launch_flux_d<2>(h))) return rc; });
   return GRMHD_OK;
 }
 
