@@ -111,9 +111,17 @@ __device__ __forceinline__ int fm_var_field(int D, int slot) {
   return slot < 5 ? F_P + slot : F_BC + (D + 1 + (slot - 5)) % 3;
 }
 
-// index of cell 0 of pencil r along D (r = flattened transverse index incl. the apron)
+// index of cell 0 of pencil r along D (r = flattened transverse index incl. the apron).
+// apron != 0: only the two apron columns t0 = -1 and t0 = n_t0 (t0 = y for D = x, else x) at
+// every t1 in [-1, n_t1] -- the pencils k_flux_tma (flux_tma.cuh) leaves out.
 template <int D>
-__device__ __forceinline__ long long fm_pencil_base(const Geom& g, int r) {
+__device__ __forceinline__ long long fm_pencil_base(const Geom& g, int r, int apron) {
+  if (apron) {
+    const int t1 = (r >> 1) - 1;
+    if (D == 0) return g.at(0, (r & 1) ? g.ny : -1, t1);
+    const int i = (r & 1) ? g.nx : -1;
+    return D == 1 ? g.at(i, 0, t1) : g.at(i, t1, 0);
+  }
   if (D == 0) {
     const int na = g.ny + 2;
     return g.at(0, r % na - 1, r / na - 1);
@@ -126,7 +134,8 @@ __device__ __forceinline__ long long fm_pencil_base(const Geom& g, int r) {
   }
 }
 
-__host__ __device__ inline int fm_npencils(const Geom& g, int D) {
+__host__ __device__ inline int fm_npencils(const Geom& g, int D, int apron) {
+  if (apron) return 2 * ((D == 2 ? g.ny : g.nz) + 2);
   return D == 0 ? (g.ny + 2) * (g.nz + 2)
                 : (D == 1 ? (g.nx + 2) * (g.nz + 2) : (g.nx + 2) * (g.ny + 2));
 }
@@ -135,7 +144,7 @@ __host__ __device__ inline int fm_npencils(const Geom& g, int D) {
 // grid: x = pencil groups, y = segments of `seglen` faces (seglen a multiple of TC).
 template <int D, int RECON, int TC>
 __global__ void __launch_bounds__(FM_THREADS, 4)
-k_flux_march(double* __restrict__ base, Geom g, Eos E, int seglen) {
+k_flux_march(double* __restrict__ base, Geom g, Eos E, int seglen, int apron) {
   using Smem = FluxSmem<D, TC>;
   extern __shared__ __align__(16) unsigned char fm_smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(fm_smem_raw);
@@ -144,14 +153,14 @@ k_flux_march(double* __restrict__ base, Geom g, Eos E, int seglen) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nD = g.n(D);
   const long long sd = D == 0 ? 1 : (D == 1 ? g.sy : g.sz);
-  const int npen = fm_npencils(g, D);
+  const int npen = fm_npencils(g, D, apron);
   const int f0 = blockIdx.y * seglen;
   const int f1 = min(f0 + seglen, nD + 1);
   const int cmax = nD + G - 1;  // last valid cell index along D
 
   // ---- phase-A identity: lane = pencil
   const int rA = min((int)blockIdx.x * 32 + lane, npen - 1);
-  const long long baseA = fm_pencil_base<D>(g, rA);
+  const long long baseA = fm_pencil_base<D>(g, rA, apron);
   const int s0 = 2 * warp, nslot = warp == 3 ? 1 : 2;
   const double* qsrc[2];
   qsrc[0] = fld(base, g, fm_var_field(D, s0)) + baseA;
@@ -202,7 +211,7 @@ k_flux_march(double* __restrict__ base, Geom g, Eos E, int seglen) {
     else { plB[it] = lane; clB[it] = warp + 4 * it; }
     const int r = (int)blockIdx.x * 32 + plB[it];
     okB[it] = r < npen;
-    baseB[it] = fm_pencil_base<D>(g, min(r, npen - 1));
+    baseB[it] = fm_pencil_base<D>(g, min(r, npen - 1), apron);
   }
   const int fid = D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ);
 

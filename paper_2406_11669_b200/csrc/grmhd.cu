@@ -12,6 +12,7 @@
 
 #include "kernels_flux.cuh"
 #include "flux_march.cuh"
+#include "flux_tma.cuh"
 #include "kernels_batch.cuh"
 
 using namespace gk;
@@ -32,6 +33,10 @@ struct grmhd {
   long long steps = 0;
   long long launches = 0;
   int fm_conc[9] = {0};  // resident blocks of each flux-kernel instantiation (0 = not queried)
+  int ft_conc[9] = {0};  // ... of the TMA-fed instantiations
+  CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][.] of the ring stages, per direction
+  bool tma_ok = false;
+  int flux_impl = 1;     // 1: k_flux_tma (+ k_flux_march on the apron columns), 0: k_flux_march
   char err[256] = {0};
   // optional per-kernel-group timing ("kernel_timing" option): CUDA events on the stream
   bool ktime = false;
@@ -274,7 +279,7 @@ int after_stage(grmhd* h, bool want_speed) {
 constexpr int FM_TC = 4;
 
 template <int D, int RECON>
-int launch_flux(grmhd* h) {
+int launch_flux(grmhd* h, int apron) {
   const Geom& g = h->g;
   auto kern = k_flux_march<D, RECON, FM_TC>;
   const int smem = (int)sizeof(FluxSmem<D, FM_TC>);
@@ -288,7 +293,7 @@ int launch_flux(grmhd* h) {
     h->fm_conc[cfg] = nb * nsm > 0 ? nb * nsm : 1;
   }
   const int nfaces = g.n(D) + 1;
-  const int ngroups = (fm_npencils(g, D) + 31) / 32;
+  const int ngroups = (fm_npencils(g, D, apron) + 31) / 32;
   // segments along D: fill whole waves of resident blocks; a segment costs ~2 extra cells
   int best = 1;
   double best_cost = 1e300;
@@ -303,17 +308,101 @@ int launch_flux(grmhd* h) {
   }
   const int seglen = ((nfaces + best - 1) / best + FM_TC - 1) / FM_TC * FM_TC;
   const int nseg = (nfaces + seglen - 1) / seglen;
-  kern<<<dim3(ngroups, nseg), FM_THREADS, smem, h->s>>>(h->base, g, h->E, seglen);
+  kern<<<dim3(ngroups, nseg), FM_THREADS, smem, h->s>>>(h->base, g, h->E, seglen, apron);
+  h->launches++;
   return GRMHD_OK;
+}
+
+// ---- TMA-fed flux kernel (flux_tma.cuh) ---------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tensor = the whole workspace as [field][z][y][x]; box of direction D with nf fields
+bool make_tensor_maps(grmhd* h) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) !=
+          cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) {
+    cudaGetLastError();
+    return false;
+  }
+  const Geom& g = h->g;
+  const cuuint64_t dims[4] = {(cuuint64_t)g.PXP, (cuuint64_t)g.PY, (cuuint64_t)g.PZ,
+                              (cuuint64_t)h->nfields};
+  const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8,
+                                 (cuuint64_t)g.NPA * 8};
+  const cuuint32_t es[4] = {1, 1, 1, 1};
+  for (int d = 0; d < 3; d++) {
+    for (int w = 0; w < 2; w++) {
+      cuuint32_t box[4] = {32, 1, 1, (cuuint32_t)(w == 0 ? FT_NMET : 1)};
+      if (d == 0) { box[0] = FT_TC; box[1] = 32; }
+      else box[d] = FT_TC;
+      CUresult r = ((EncodeTiledFn)fn)(w == 0 ? &h->tm_met[d] : &h->tm_bf[d],
+                                       CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, h->base, dims, strides,
+                                       box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) return false;
+    }
+  }
+  return true;
+}
+
+template <int D, int RECON>
+int launch_flux_tma(grmhd* h) {
+  const Geom& g = h->g;
+  auto kern = k_flux_tma<D, RECON>;
+  const int smem = (int)sizeof(FtSmem<D>);
+  const int cfg = D * 3 + RECON;
+  if (h->ft_conc[cfg] == 0) {
+    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int nb = 0, dev = 0, nsm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, FT_THREADS, smem));
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    h->ft_conc[cfg] = nb * nsm > 0 ? nb * nsm : 1;
+  }
+  const int nt0 = D == 0 ? g.ny : g.nx, nt1 = D == 2 ? g.ny : g.nz;
+  const int ngx = (nt0 + 31) / 32;
+  const long long ngroups = (long long)ngx * (nt1 + 2);
+  const int nfaces = g.n(D) + 1 + (D == 0 ? 2 : 0);  // D = x marches from face -2 (alignment)
+  int best = 1;
+  double best_cost = 1e300;
+  for (int ns = 1; ns <= 64; ns++) {
+    const int sl = ((nfaces + ns - 1) / ns + FT_TC - 1) / FT_TC * FT_TC;
+    if (ns > 1 && sl < 16) break;
+    const int nseg = (nfaces + sl - 1) / sl;
+    const long long nblk = (long long)nseg * ngroups;
+    const long long waves = (nblk + h->ft_conc[cfg] - 1) / h->ft_conc[cfg];
+    const double cost = (double)waves * (sl + 3);
+    if (cost < best_cost * 0.97) { best_cost = cost; best = ns; }
+  }
+  const int seglen = ((nfaces + best - 1) / best + FT_TC - 1) / FT_TC * FT_TC;
+  const int nseg = (nfaces + seglen - 1) / seglen;
+  kern<<<dim3((unsigned)ngroups, nseg), FT_THREADS, smem, h->s>>>(h->base, g, h->E, seglen, ngx,
+                                                                  h->tm_met[D], h->tm_bf[D]);
+  h->launches++;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_tma");
+  return launch_flux<D, RECON>(h, 1);  // the two apron columns along t0
 }
 
 template <int D>
 int launch_flux_d(grmhd* h) {
   const int recon = h->o.recon == 0 ? 0 : (h->o.ppm_flatten ? 2 : 1);
-  int rc = recon == 0 ? launch_flux<D, 0>(h) : (recon == 1 ? launch_flux<D, 1>(h)
-                                                            : launch_flux<D, 2>(h));
+  const int nt0 = D == 0 ? h->g.ny : h->g.nx;
+  int rc;
+  if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
+    rc = recon == 0 ? launch_flux_tma<D, 0>(h)
+                    : (recon == 1 ? launch_flux_tma<D, 1>(h) : launch_flux_tma<D, 2>(h));
+  else
+    rc = recon == 0 ? launch_flux<D, 0>(h, 0)
+                    : (recon == 1 ? launch_flux<D, 1>(h, 0) : launch_flux<D, 2>(h, 0));
   if (rc) return rc;
-  CKL("k_flux_march");
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_march");
   return GRMHD_OK;
 }
 
@@ -421,6 +510,7 @@ int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3], const g
     delete h;
     return GRMHD_ECUDA;
   }
+  h->tma_ok = make_tensor_maps(h);
   *out = h;
   return GRMHD_OK;
 }
@@ -588,6 +678,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (!h || !key) return GRMHD_EINVAL;
   if (std::strcmp(key, "fixed_dt") == 0) {
     h->fixed_dt = value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "flux_kernel") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
+    h->flux_impl = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "kernel_timing") == 0) {
