@@ -111,12 +111,26 @@ __device__ __forceinline__ double ft_sqrt(double x) {
 }
 
 // ---- branch-free reconstruction state of one variable on one pencil -------------------------
-// G8(a): monotonised-central slope from the two one-sided differences.
+// min / max as one compare + select (no NaN bookkeeping: operands are finite by construction)
+__device__ __forceinline__ double ft_min(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double ft_max(double a, double b) { return a > b ? a : b; }
+
+// select that stays a select (the compiler turns ?: chains of the limiter into branches)
+__device__ __forceinline__ double ft_sel(bool c, double a, double b) {
+  double r;
+  asm("{\n.reg .pred p;\nsetp.ne.s32 p, %3, 0;\nselp.f64 %0, %1, %2, p;\n}"
+      : "=d"(r) : "d"(a), "d"(b), "r"((int)c));
+  return r;
+}
+
+// G8(a): monotonised-central slope from the two one-sided differences.  For same-signed
+// dm, dp the candidates d = (dp+dm)/2 and 2 min(|dp|,|dm|) carry the sign of d already.
 __device__ __forceinline__ double ft_slope(double dm, double dp) {
   const double d = 0.5 * (dp + dm);
-  const double lim = fmin(fabs(d), 2.0 * fmin(fabs(dp), fabs(dm)));
-  const double s = copysign(lim, d);
-  return dp * dm > 0.0 ? s : 0.0;
+  const double m = fabs(dp) < fabs(dm) ? dp : dm;
+  const double m2 = m + m;
+  const double r = fabs(d) < fabs(m2) ? d : m2;
+  return dp * dm > 0.0 ? r : 0.0;
 }
 
 template <int RECON>
@@ -145,8 +159,8 @@ struct FtMarch {
     const double dr = qb - qa;
     if (RECON == 0) {
       // G7
-      const double m = fmin(fabs(dl), fabs(dr));
-      const double s = dl * dr > 0.0 ? copysign(m, dl) : 0.0;
+      const double m = fabs(dl) < fabs(dr) ? dl : dr;
+      const double s = dl * dr > 0.0 ? m : 0.0;
       qm = fma(-0.5, s, qa);
       qp = fma(0.5, s, qa);
     } else {
@@ -168,8 +182,13 @@ struct FtMarch {
       const bool fixp = aa > 2.0 * ab;
       const double qm2 = fma(-2.0, a, qa);
       const double qp2 = fma(2.0, b, qa);
+#ifndef FT_NO_SELP
+      qm = ft_sel(flat, qa, ft_sel(fixm, qm2, qm));
+      qp = ft_sel(flat, qa, ft_sel(fixp, qp2, qp));
+#else
       qm = flat ? qa : (fixm ? qm2 : qm);
       qp = flat ? qa : (fixp ? qp2 : qp);
+#endif
       s0 = dmn; il = ir;
     }
     dl = dr; qa = qb; qb = qn;
@@ -187,11 +206,11 @@ struct FtFlat {
   __device__ __forceinline__ double step(double pn, double vn) {
     const double dp1 = pp1 - pm1;
     const double dp2 = pn - pm2;
-    const bool on = fabs(dp1) > 0.33 * fmin(pp1, pm1) && vm1 > vn;
+    const bool on = fabs(dp1) > 0.33 * ft_min(pp1, pm1) && vm1 > vn;
     const bool z = dp2 == 0.0;
     const double r = ft_rcp(z ? 1.0 : dp2);
     double f = 10.0 * fma(dp1, r, -0.75);
-    f = fmin(1.0, fmax(0.0, f));
+    f = ft_min(1.0, ft_max(0.0, f));
     f = z ? 1.0 : f;
     pm2 = pm1; pm1 = p0; p0 = pp1; pp1 = pn;
     vm1 = v0; v0 = vn;
@@ -268,6 +287,30 @@ __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double
   const double bd = D == 0 ? M.bx : (D == 1 ? M.by : M.bz);
   lm = aod * (mid - root) - bd;
   lp = aod * (mid + root) - bd;
+}
+
+// R7 (eq. 29 / eq. 30): out[r] = sqrt(gamma_f) * F^[r]
+__device__ __forceinline__ void ft_hll(const double UL[7], const double GL[7], double lmL,
+                                       double lpL, const double UR[7], const double GR[7],
+                                       double lmR, double lpR, double sgf, int riemann,
+                                       double out[7]) {
+  const double cmax = ft_max(0.0, ft_max(lpL, lpR));
+  const double cmin = -ft_min(0.0, ft_min(lmL, lmR));
+  const double cs = cmax + cmin;
+  if (riemann == 1) {  // eq. (30)
+    const double cw = ft_max(cmax, cmin);
+    const double hs = 0.5 * sgf;
+#pragma unroll
+    for (int r = 0; r < 7; r++) out[r] = hs * (GR[r] + GL[r] - cw * (UR[r] - UL[r]));
+  } else {  // eq. (29); c_max + c_min < 1e-300: plain average
+    const bool deg = cs < 1e-300;
+    const double w = sgf * ft_rcp(deg ? 1.0 : cs);
+    const double a = deg ? 0.5 * sgf : cmin * w;
+    const double b = deg ? 0.5 * sgf : cmax * w;
+    const double cc = deg ? 0.0 : cmax * cmin * w;
+#pragma unroll
+    for (int r = 0; r < 7; r++) out[r] = a * GR[r] + b * GL[r] - cc * (UR[r] - UL[r]);
+  }
 }
 
 // 32-byte global load of 4 consecutive doubles (address 32-byte aligned)
@@ -490,7 +533,7 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
                  D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]),
                  M, gdd, E, UR, GR, lmR, lpR);
       double out[7];
-      hll_rows(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
+      ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
       if (okB && f >= 0 && f < f1) {
         double* o = outp + f * sd;
 #pragma unroll
