@@ -187,9 +187,11 @@ def config_name(args):
 ALG_BYTES = {  # algorithmic bytes per interior cell and launch
     "flux_x": FLUX_BYTES_PER_CELL_DIR, "flux_y": FLUX_BYTES_PER_CELL_DIR,
     "flux_z": FLUX_BYTES_PER_CELL_DIR,
-    "update": (49 + 5 + 12 + 3) * 8,      # hydro update 49 r + 5 w, EMF/A update 12 r + 3 w
-    "bfield": (3 + 3 + 6 + 6) * 8,        # A (3) + B~0 (3) + gamma (6) read, B~ (3) + B_c (3) written
-    "con2prim": (5 + 3 + 6 + 5) * 8,      # U~ (5) + B_c (3) + gamma (6) read, P (5) written
+    # update: fluxes 15 + 6, sources 4, Y 8, Y0 8 read; Y 8 written
+    "update": (21 + 4 + 8 + 8 + 8) * 8,
+    # fused post-update kernel (curl A, con2prim, sources, max speed): A 3, B~0 3, metric 16,
+    # U~ 5 read; B~ 3, B_c 3, P 5, sources 4 written
+    "con2prim": (3 + 3 + 16 + 5 + 3 + 3 + 5 + 4) * 8,
 }
 
 

@@ -78,42 +78,7 @@ __device__ __forceinline__ void ft_tma_4d(void* dst, const CUtensorMap* tm,
       : "memory");
 }
 
-// ---- special functions without special-case paths ----------------------------------------
-// 1/x: hardware seed (2^-23) + two Newton steps; x normal, finite, non-zero.
-__device__ __forceinline__ double ft_rcp(double x) {
-  double r;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  e = fma(-x, r, 1.0);
-  r = fma(r, e, r);
-  return r;
-}
-// x^(-1/2): hardware seed + two Newton steps (y <- y + y/2 (1 - x y^2)); x normal, > 0.
-__device__ __forceinline__ double ft_rsqrt(double x) {
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double t = x * y;
-  double e = fma(-t, y, 1.0);
-  y = fma(0.5 * y, e, y);
-  t = x * y;
-  e = fma(-t, y, 1.0);
-  y = fma(0.5 * y, e, y);
-  return y;
-}
-// sqrt(x) for x >= 0 (0 below 1e-280): s = x y, one correction step with the residual.
-__device__ __forceinline__ double ft_sqrt(double x) {
-  const double y = ft_rsqrt(x);
-  double s = x * y;
-  const double r = fma(-s, s, x);
-  s = fma(0.5 * y, r, s);
-  return x > 1e-280 ? s : 0.0;
-}
-
 // ---- branch-free reconstruction state of one variable on one pencil -------------------------
-// min / max as one compare + select (no NaN bookkeeping: operands are finite by construction)
-__device__ __forceinline__ double ft_min(double a, double b) { return a < b ? a : b; }
-__device__ __forceinline__ double ft_max(double a, double b) { return a > b ? a : b; }
 
 // select that stays a select (the compiler turns ?: chains of the limiter into branches)
 __device__ __forceinline__ double ft_sel(bool c, double a, double b) {

@@ -259,14 +259,11 @@ int after_stage(grmhd* h, bool want_speed) {
   KT(KG_BFIELD, {
     rc = fill_ghosts(h, fill_vecpot());
     if (rc) return rc;
-    k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
-        h->base, g);
-    CKL("k_bfield");
   });
   KT(KG_C2P, {
-    k_con2prim<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(
+    k_post<false><<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
         h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
-    CKL("k_con2prim");
+    CKL("k_post");
   });
   KT(KG_GHOST, {
     rc = fill_ghosts(h, fill_prims());
@@ -433,8 +430,8 @@ int one_step(grmhd* h) {
     int rc = compute_fluxes(h);
     if (rc) return rc;
     KT(KG_UPDATE, {
-      k_update<<<grd3(g.nx + 1, g.ny + 1, g.nz + 1), blk3(), 0, h->s>>>(h->base, g, h->E,
-                                                                       h->dst, st[s]);
+      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, g.nz + 1), dim3(128, 2, 1), 0,
+                 h->s>>>(h->base, g, h->dst, st[s]);
       CKL("k_update");
     });
     rc = after_stage(h, s == ns - 1);
@@ -453,15 +450,11 @@ int init_state(grmhd* h) {
   const Geom& g = h->g;
   int rc = fill_ghosts(h, fill_vecpot());
   if (rc) return rc;
-  k_bfield<<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
-      h->base, g);
-  CKL("k_bfield");
-  k_prim2con<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(h->base, g, h->E);
-  CKL("k_prim2con");
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 0);
   CKL("k_reset_state");
-  k_maxspeed<<<grd3(g.nx, g.ny, g.nz), blk3(), 0, h->s>>>(h->base, g, h->E, h->dst);
-  CKL("k_maxspeed");
+  k_post<true><<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+      h->base, nullptr, g, h->E, h->dst, 1);
+  CKL("k_post");
   return GRMHD_OK;
 }
 

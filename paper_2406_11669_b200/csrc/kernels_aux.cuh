@@ -253,7 +253,7 @@ __device__ __forceinline__ void block_max3_atomic(double m0, double m1, double m
 // R16: max(|lambda_-|, |lambda_+|) per direction at a cell centre
 __device__ __forceinline__ void cell_speeds(const Prim& P, const Met& M, const Eos& E,
                                             double s[3]) {
-  const double idet = 1.0 / det_gamma(M);
+  const double idet = ft_rcp(det_gamma(M));
   const Pt pt = point_state(P, M, E);
   double lm, lp;
   char_speeds<0>(P, pt, M, inv_gamma_dd<0>(M, idet), E, lm, lp);
@@ -352,6 +352,149 @@ __global__ void k_prim2con(double* __restrict__ base, Geom g, Eos E) {
   prim2con(load_prim(base, g, c), M, E, U);
 #pragma unroll
   for (int r = 0; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
+}
+
+// ------------------------------------------------------------ fused post-update kernel
+// 4th-order centred derivative (G12); this operand order gives exactly 0 on constants
+__device__ __forceinline__ double d4(const double* __restrict__ q, int c, int sd, double i12dx) {
+  return (8.0 * (q[c + sd] - q[c - sd]) - (q[c + 2 * sd] - q[c - 2 * sd])) * i12dx;
+}
+
+// R9 / G11: alpha sqrt(gamma) S for the rows S_x, S_y, S_z, tau at an interior cell
+// (eq. (19) PAPER.md:125 in 3+1 form; metric derivatives PAPER.md:384)
+__device__ __forceinline__ void cell_sources(const double* __restrict__ base, const Geom& g, int c,
+                                             const Prim& P, const Met& M, double sg,
+                                             const Eos& E, double S[4]) {
+  const SrcCoef sc = source_coef(P, M, E);
+  // S_tau, curvature part: 2 C^{ik} K_ik
+  double St = 2.0 * contract(sc.C, fld(base, g, F_MET + 10)[c], fld(base, g, F_MET + 11)[c],
+                             fld(base, g, F_MET + 12)[c], fld(base, g, F_MET + 13)[c],
+                             fld(base, g, F_MET + 14)[c], fld(base, g, F_MET + 15)[c]);
+  const double asg = M.a * sg;
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const int sd = a == 0 ? 1 : (a == 1 ? (int)g.sy : (int)g.sz);
+    const double w = g.idx[a] * (1.0 / 12.0);
+    const double da = d4(fld(base, g, F_MET + 0), c, sd, w);
+    const double dbx = d4(fld(base, g, F_MET + 1), c, sd, w);
+    const double dby = d4(fld(base, g, F_MET + 2), c, sd, w);
+    const double dbz = d4(fld(base, g, F_MET + 3), c, sd, w);
+    const double cg = contract(sc.C, d4(fld(base, g, F_MET + 4), c, sd, w),
+                               d4(fld(base, g, F_MET + 5), c, sd, w),
+                               d4(fld(base, g, F_MET + 6), c, sd, w),
+                               d4(fld(base, g, F_MET + 7), c, sd, w),
+                               d4(fld(base, g, F_MET + 8), c, sd, w),
+                               d4(fld(base, g, F_MET + 9), c, sd, w));
+    S[a] = asg * (cg - sc.T00a * da + sc.T0lx * dbx + sc.T0ly * dby + sc.T0lz * dbz);
+    St -= (a == 0 ? sc.ax : (a == 1 ? sc.ay : sc.az)) * da;
+  }
+  S[3] = asg * St;
+}
+
+// After a change of (U~, A) (an RK stage) or of the initial data: one pass that
+//   R13  builds B~ = B~0 + curl A on the lower faces of every padded index and the
+//        cell-centred B^i (mean of the two faces / sqrt(gamma)),
+//   R14  recovers the primitives of the interior cells (INIT: takes the given primitives
+//        and forms U~ = sqrt(gamma) U(P, B_c) instead, eqs (20)-(22)),
+//   R9   stores alpha sqrt(gamma) S of those primitives for the next k_update,
+//   R16  accumulates the max characteristic speeds when want_speed.
+// One thread per padded index (i,j,k) in [-G, n+G].
+template <bool INIT>
+__global__ void __launch_bounds__(128, 4)
+k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
+       DevState* __restrict__ st, int want_speed) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - G;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y - G;
+  const int k = blockIdx.z - G;
+  const bool inpad = i <= g.nx + G && j <= g.ny + G;
+  const int c = (int)g.at(min(i, g.nx + G), min(j, g.ny + G), k);
+  const bool ix = i < g.nx + G, jy = j < g.ny + G, kz = k < g.nz + G;
+  double Bx = 0.0, By = 0.0, Bz = 0.0;
+  Met M;
+  double sg = 1.0;
+  if (inpad) {
+    const double* Ax = fld(base, g, F_Y + 5);
+    const double* Ay = fld(base, g, F_Y + 6);
+    const double* Az = fld(base, g, F_Y + 7);
+    const double* B0x = fld(base, g, F_B0 + 0);
+    const double* B0y = fld(base, g, F_B0 + 1);
+    const double* B0z = fld(base, g, F_B0 + 2);
+    const double bx = (jy && kz) ? face_bx(Ay, Az, B0x, g, c) : B0x[c];
+    const double by = (ix && kz) ? face_by(Ax, Az, B0y, g, c) : B0y[c];
+    const double bz = (ix && jy) ? face_bz(Ax, Ay, B0z, g, c) : B0z[c];
+    fld(base, g, F_BF + 0)[c] = bx;
+    fld(base, g, F_BF + 1)[c] = by;
+    fld(base, g, F_BF + 2)[c] = bz;
+    if (ix && jy && kz) {
+      M = load_met(base, g, c);
+      const double det = det_gamma(M);
+      const double isg = ft_rsqrt(det);
+      sg = det * isg;
+      Bx = 0.5 * (bx + face_bx(Ay, Az, B0x, g, c + 1)) * isg;
+      By = 0.5 * (by + face_by(Ax, Az, B0y, g, c + g.sy)) * isg;
+      Bz = 0.5 * (bz + face_bz(Ax, Ay, B0z, g, c + g.sz)) * isg;
+      fld(base, g, F_BC + 0)[c] = Bx;
+      fld(base, g, F_BC + 1)[c] = By;
+      fld(base, g, F_BC + 2)[c] = Bz;
+    }
+  }
+  const bool in = i >= 0 && i < g.nx && j >= 0 && j < g.ny && k >= 0 && k < g.nz;
+  double s[3] = {0.0, 0.0, 0.0};
+  int bits = 0, iters = 0;
+  if (in) {
+    double P5[5];
+    if (INIT) {
+#pragma unroll
+      for (int r = 0; r < 5; r++) P5[r] = fld(base, g, F_P + r)[c];
+      const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
+      double U[5];
+      prim2con(P, M, E, U);
+#pragma unroll
+      for (int r = 0; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
+    } else {
+      const double isg = ft_rcp(sg);
+      double U[5];
+#pragma unroll
+      for (int r = 0; r < 5; r++) U[r] = fld(base, g, F_Y + r)[c] * isg;  // undensitise, eq. (17)
+      int rewrite;
+      bits = con2prim(U, Bx, By, Bz, M, E, mask != nullptr && mask[c] != 0, P5, iters, rewrite);
+#pragma unroll
+      for (int r = 0; r < 5; r++) fld(base, g, F_P + r)[c] = P5[r];
+      if (rewrite & 1) fld(base, g, F_Y + 0)[c] = sg * U[0];
+      if (rewrite & 2) {
+#pragma unroll
+        for (int r = 1; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
+      }
+    }
+    const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
+    double S[4];
+    cell_sources(base, g, c, P, M, sg, E, S);
+#pragma unroll
+    for (int r = 0; r < 4; r++) fld(base, g, F_SRC + r)[c] = S[r];
+    if (want_speed) cell_speeds(P, M, E, s);
+  }
+  if (!INIT) {
+    // counters: integer sums and maxima, order independent
+    const unsigned any = __ballot_sync(0xffffffffu, bits != 0);
+    if (any) {
+      const int nf = __popc(__ballot_sync(0xffffffffu, (bits & 2) != 0));
+      const int np = __popc(__ballot_sync(0xffffffffu, (bits & 4) != 0));
+      const int na = __popc(__ballot_sync(0xffffffffu, (bits & 1) != 0));
+      const int nw = __popc(__ballot_sync(0xffffffffu, (bits & 8) != 0));
+      if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) {
+        if (nf) atomicAdd((unsigned long long*)&st->c2p_fail, (unsigned long long)nf);
+        if (np) atomicAdd((unsigned long long*)&st->p_fix, (unsigned long long)np);
+        if (na) atomicAdd((unsigned long long*)&st->atmo, (unsigned long long)na);
+        if (nw) atomicAdd((unsigned long long*)&st->w_cap, (unsigned long long)nw);
+      }
+    }
+    int mi = iters;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mi = max(mi, __shfl_xor_sync(0xffffffffu, mi, o));
+    if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0 && mi > 0)
+      atomicMax((long long*)&st->c2p_maxiter, (long long)mi);
+  }
+  if (want_speed) block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
 }
 
 // ---------------------------------------------------------------------------------- dt

@@ -1,5 +1,5 @@
 // kernels_flux.cuh -- reconstruction + Riemann flux per direction (A3+A4) and the
-// divergence + source + flux-CT + RK update (A5, A6, A7).
+// divergence + flux-CT + RK update (A5, A6, A7; the sources of A5 are evaluated in k_post).
 #pragma once
 #include "kernels_aux.cuh"
 
@@ -101,16 +101,12 @@ __device__ __forceinline__ void rk_apply(double* __restrict__ base, const Geom& 
   }
 }
 
-__device__ __forceinline__ double d4(const double* __restrict__ q, long long c, long long sd,
-                                     double i12dx) {
-  // 4th-order centred derivative (G12); this operand order gives exactly 0 on constants
-  return (8.0 * (q[c + sd] - q[c - sd]) - (q[c + 2 * sd] - q[c - 2 * sd])) * i12dx;
-}
-
 // One thread per index (i,j,k) in [0,nx]x[0,ny]x[0,nz]: the cell's hydro update (if it is
-// an interior cell) and the three edges attached to it in the lower convention.
-__global__ void __launch_bounds__(128)
-k_update(double* __restrict__ base, Geom g, Eos E, const DevState* __restrict__ st, RkStage rk) {
+// an interior cell) and the three edges attached to it in the lower convention.  The
+// sources alpha sqrt(gamma) S were stored by k_post (kernels_aux.cuh) when the primitives
+// they depend on were recovered, so this kernel only streams: fluxes, sources, Y, Y0.
+__global__ void __launch_bounds__(256, 3)
+k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z;
@@ -121,32 +117,6 @@ k_update(double* __restrict__ base, Geom g, Eos E, const DevState* __restrict__ 
 
   if (i < g.nx && j < g.ny && k < g.nz) {
     // R8: L(U~) = -sum_d (F~_{i+1/2} - F~_{i-1/2})/dx_d + alpha sqrt(gamma) S, eq. (17)
-    const Met M = load_met(base, g, c);
-    const Prim P = load_prim(base, g, c);
-    const SrcCoef sc = source_coef(P, M, E);
-    const double asg = M.a * sqrt(det_gamma(M));
-    double S[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    // S_tau, curvature part: 2 C^{ik} K_ik
-    S[4] = 2.0 * contract(sc.C, fld(base, g, F_MET + 10)[c], fld(base, g, F_MET + 11)[c],
-                          fld(base, g, F_MET + 12)[c], fld(base, g, F_MET + 13)[c],
-                          fld(base, g, F_MET + 14)[c], fld(base, g, F_MET + 15)[c]);
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-      const long long sd = a == 0 ? 1 : (a == 1 ? sy : sz);
-      const double w = g.idx[a] * (1.0 / 12.0);
-      const double da = d4(fld(base, g, F_MET + 0), c, sd, w);
-      const double dbx = d4(fld(base, g, F_MET + 1), c, sd, w);
-      const double dby = d4(fld(base, g, F_MET + 2), c, sd, w);
-      const double dbz = d4(fld(base, g, F_MET + 3), c, sd, w);
-      const double cg = contract(sc.C, d4(fld(base, g, F_MET + 4), c, sd, w),
-                                 d4(fld(base, g, F_MET + 5), c, sd, w),
-                                 d4(fld(base, g, F_MET + 6), c, sd, w),
-                                 d4(fld(base, g, F_MET + 7), c, sd, w),
-                                 d4(fld(base, g, F_MET + 8), c, sd, w),
-                                 d4(fld(base, g, F_MET + 9), c, sd, w));
-      S[1 + a] = cg - sc.T00a * da + sc.T0lx * dbx + sc.T0ly * dby + sc.T0lz * dbz;
-      S[4] -= (a == 0 ? sc.ax : (a == 1 ? sc.ay : sc.az)) * da;
-    }
 #pragma unroll
     for (int r = 0; r < 5; r++) {
       const double* Fx = fld(base, g, F_FX + r);
@@ -155,7 +125,8 @@ k_update(double* __restrict__ base, Geom g, Eos E, const DevState* __restrict__ 
       double div = (Fx[c + 1] - Fx[c]) * g.idx[0];
       div += (Fy[c + sy] - Fy[c]) * g.idx[1];
       div += (Fz[c + sz] - Fz[c]) * g.idx[2];
-      rk_apply(base, g, r, c, -div + asg * S[r], h, rk);
+      const double src = r == 0 ? 0.0 : fld(base, g, F_SRC + r - 1)[c];  // S_D = 0
+      rk_apply(base, g, r, c, -div + src, h, rk);
     }
   }
   // R10 (flux-CT, G13/G14) and R11 (d_t A_i = -E_i).  Stored B rows:

@@ -45,9 +45,10 @@ enum FieldId {
   F_FX = 46,    // 7 : stored x-fluxes: D,S_x,S_y,S_z,tau rows + B^y, B^z rows
   F_FY = 53,    // 7 : y-fluxes (+ B^z, B^x rows)
   F_FZ = 60,    // 7 : z-fluxes (+ B^x, B^y rows)
-  F_KS = 67,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
-  F_END_RK23 = 67,
-  F_END_RK4 = 75
+  F_SRC = 67,   // 4 : alpha sqrt(gamma) S of eq. (19) for the rows S_x, S_y, S_z, tau (cells)
+  F_KS = 71,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
+  F_END_RK23 = 71,
+  F_END_RK4 = 79
 };
 
 // device-resident scalars of a handle

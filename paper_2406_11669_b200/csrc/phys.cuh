@@ -40,6 +40,39 @@ struct Eos {
 
 __device__ __forceinline__ double sq(double x) { return x * x; }
 
+// ---- special functions without special-case paths ----------------------------------------
+// 1/x: hardware seed (2^-23) + two Newton steps; x normal, finite, non-zero.
+__device__ __forceinline__ double ft_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  return r;
+}
+// x^(-1/2): hardware seed + two Newton steps (y <- y + y/2 (1 - x y^2)); x normal, > 0.
+__device__ __forceinline__ double ft_rsqrt(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = x * y;
+  double e = fma(-t, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  t = x * y;
+  e = fma(-t, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  return y;
+}
+// sqrt(x) for x >= 0 (0 below 1e-280): s = x y, one correction step with the residual.
+__device__ __forceinline__ double ft_sqrt(double x) {
+  const double y = ft_rsqrt(x);
+  double s = x * y;
+  const double r = fma(-s, s, x);
+  s = fma(0.5 * y, r, s);
+  return x > 1e-280 ? s : 0.0;
+}
+
+
 __device__ __forceinline__ double det_gamma(const Met& M) {
   return M.gxx * (M.gyy * M.gzz - M.gyz * M.gyz) - M.gxy * (M.gxy * M.gzz - M.gyz * M.gxz) +
          M.gxz * (M.gxy * M.gyz - M.gyy * M.gxz);
@@ -75,6 +108,10 @@ __device__ __forceinline__ void lower(const Met& M, double x, double y, double z
   lz = M.gxz * x + M.gyz * y + M.gzz * z;
 }
 
+// min / max as one compare + select (no NaN bookkeeping)
+__device__ __forceinline__ double ft_min(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double ft_max(double a, double b) { return a > b ? a : b; }
+
 // ---------------------------------------------------------------------------------------
 // Point state shared by eqs (13), (20)-(22), (37): PAPER.md:102, 129-133, 266.
 struct Pt {
@@ -90,7 +127,7 @@ __device__ __forceinline__ Pt point_state(const Prim& P, const Met& M, const Eos
   const double B2 = Blx * P.Bx + Bly * P.By + Blz * P.Bz;
   const double Bv = P.Bx * s.vlx + P.By * s.vly + P.Bz * s.vlz;
   const double iW2 = 1.0 - s.v2;
-  s.W = rsqrt(iW2);                  // W = (1 - v^2)^(-1/2)
+  s.W = ft_rsqrt(iW2);               // W = (1 - v^2)^(-1/2)
   s.iW = iW2 * s.W;                  // 1/W
   s.ab0 = s.W * Bv;                  // alpha b^0 = W B^i v_i, eq. (13)
   s.b2 = (B2 + s.ab0 * s.ab0) * iW2; // b^2 = (B^2 + (alpha b^0)^2)/W^2, eq. (13)
@@ -120,14 +157,14 @@ __device__ __forceinline__ void char_speeds(const Prim& P, const Pt& s, const Me
                                             const Eos& E, double& lm, double& lp) {
   const double e = s.rhoh + s.b2;
   const double Gp = E.Gamma * P.p;
-  const double a2 = (Gp * e + s.b2 * (s.rhoh - Gp)) / (s.rhoh * e);
+  const double a2 = (Gp * e + s.b2 * (s.rhoh - Gp)) * ft_rcp(s.rhoh * e);
   const double vd = D == 0 ? P.vx : (D == 1 ? P.vy : P.vz);
   const double bd = D == 0 ? M.bx : (D == 1 ? M.by : M.bz);
   const double den = 1.0 - s.v2 * a2;
   double rad = a2 * (1.0 - s.v2) * (gdd * den - vd * vd * (1.0 - a2));
   rad = rad < 0.0 ? 0.0 : rad;
-  const double root = sqrt(rad);
-  const double aoden = M.a / den;
+  const double root = ft_sqrt(rad);
+  const double aoden = M.a * ft_rcp(den);
   const double mid = vd * (1.0 - a2);
   lm = aoden * (mid - root) - bd;
   lp = aoden * (mid + root) - bd;

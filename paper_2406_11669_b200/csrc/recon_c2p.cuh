@@ -98,7 +98,7 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
   if (atmo) bits = 1;
   double rho = 0, vx = 0, vy = 0, vz = 0, p = 0;
   if (!atmo) {
-    const double idet = 1.0 / det_gamma(M);
+    const double idet = ft_rcp(det_gamma(M));
     const Sym3 gu = inv_gamma(M, idet);
     const double Sx = U[1], Sy = U[2], Sz = U[3];
     const double Sux = gu.xx * Sx + gu.xy * Sy + gu.xz * Sz;  // S^i
@@ -112,12 +112,14 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
     const double BS2 = BS * BS;
     const double g1 = E.gm1oG;
     double z = tau + D, v2 = 0.0;  // G17: stateless initial guess
+    double iz = ft_rcp(z);         // 1/z, carried from the convergence test of the last iterate
     bool conv = false;
     for (int it = 1; it <= E.c2p_maxit; it++) {
       iters = it;
-      const double sw = sqrt(1.0 - v2);  // 1/W
-      const double pz = g1 * (z * (1.0 - v2) - D * sw);
-      const double iz = 1.0 / z;
+      const double omv = 1.0 - v2;
+      const double W = ft_rsqrt(omv);
+      const double sw = omv * W;  // 1/W
+      const double pz = g1 * (z * omv - D * sw);
       const double iz2 = iz * iz, BS2iz3 = BS2 * iz2 * iz;
       const double B2z = B2 + z;
       // eqs (40a), (40b) and their Jacobian
@@ -125,15 +127,17 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
       const double f2 = tau + D - 0.5 * B2 * (1.0 + v2) + 0.5 * BS2 * iz2 - z + pz;
       const double J11 = 2.0 * B2z * (v2 + BS2iz3);
       const double J12 = B2z * B2z;
-      const double J21 = -BS2iz3 - 1.0 + g1 * (1.0 - v2);
-      const double J22 = -0.5 * B2 + g1 * (-z + D / (2.0 * sw));
-      const double idetJ = 1.0 / (J11 * J22 - J12 * J21);
+      const double J21 = -BS2iz3 - 1.0 + g1 * omv;
+      const double J22 = -0.5 * B2 + g1 * (0.5 * D * W - z);
+      const double idetJ = ft_rcp(J11 * J22 - J12 * J21);
       const double dz = (f2 * J12 - f1 * J22) * idetJ;
       const double dv = (f1 * J21 - f2 * J11) * idetJ;
       const double zn = fabs(z + dz);
-      const double vn = fmin(fmax(v2 + dv, 0.0), 1.0 - 1e-12);  // G18
-      const double err = fabs(dz) / zn + fabs(dv);
-      z = zn; v2 = vn;
+      const double vs = v2 + dv;
+      const double vn = ft_min(ft_max(vs, 0.0), 1.0 - 1e-12);  // G18
+      const double izn = ft_rcp(zn);
+      const double err = fabs(dz) * izn + fabs(dv);
+      z = zn; v2 = vn; iz = izn;
       if (!isfinite(err)) break;
       if (err < E.c2p_tol) { conv = true; break; }
     }
@@ -142,14 +146,15 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
     } else {
       // eqs (41a)-(41d); G19: the 1/gamma of (41d) is 1/Gamma
       const double iW2 = 1.0 - v2;
-      const double iW = sqrt(iW2);
+      const double iW = iW2 * ft_rsqrt(iW2);
       rho = D * iW;
-      const double izB = 1.0 / (z + B2);
-      const double BSz = BS / z;
+      const double izB = ft_rcp(z + B2);
+      const double BSz = BS * iz;
       vx = (Sux + BSz * Bx) * izB;
       vy = (Suy + BSz * By) * izB;
       vz = (Suz + BSz * Bz) * izB;
-      const double eps = (z * iW2 / rho - 1.0) / E.Gamma;
+      // z (1 - v^2)/rho = z/(D W)
+      const double eps = (z * iW * ft_rcp(D) - 1.0) * (1.0 - E.gm1oG);
       p = (E.Gamma - 1.0) * rho * eps;
       if (!isfinite(rho) || !isfinite(p) || !isfinite(vx) || !isfinite(vy) || !isfinite(vz) ||
           rho < E.rho_atm) {
@@ -200,8 +205,8 @@ struct SrcCoef {
 
 __device__ __forceinline__ SrcCoef source_coef(const Prim& P, const Met& M, const Eos& E) {
   const Pt s = point_state(P, M, E);
-  const double ia = 1.0 / M.a, ia2 = ia * ia;
-  const double idet = 1.0 / det_gamma(M);
+  const double ia = ft_rcp(M.a), ia2 = ia * ia;
+  const double idet = ft_rcp(det_gamma(M));
   const Sym3 gu = inv_gamma(M, idet);
   // four-velocity and comoving field, eq. (13)
   const double u0 = s.W * ia;
