@@ -177,6 +177,10 @@ bool is_device_ptr(const void* p) {
 
 dim3 blk3() { return dim3(32, 4, 1); }
 dim3 grd3(int ex, int ey, int ez) { return dim3((ex + 31) / 32, (ey + 3) / 4, ez); }
+dim3 grd_post(const Geom& g) {
+  return dim3((g.nx + 2 * G + 1 + 31) / 32, (g.ny + 2 * G + 1 + KP_BY - 1) / KP_BY,
+              (g.nz + 2 * G + 1 + KP_BZ - 1) / KP_BZ);
+}
 int grd1(long long n) {
   long long b = (n + 255) / 256;
   return (int)(b > 65535 * 16 ? 65535 * 16 : (b < 1 ? 1 : b));
@@ -261,7 +265,7 @@ int after_stage(grmhd* h, bool want_speed) {
     if (rc) return rc;
   });
   KT(KG_C2P, {
-    k_post<false><<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+    k_post<false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
         h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
     CKL("k_post");
   });
@@ -430,7 +434,7 @@ int one_step(grmhd* h) {
     int rc = compute_fluxes(h);
     if (rc) return rc;
     KT(KG_UPDATE, {
-      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, g.nz + 1), dim3(128, 2, 1), 0,
+      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 8 * (g.nz + 1)), dim3(128, 2, 1), 0,
                  h->s>>>(h->base, g, h->dst, st[s]);
       CKL("k_update");
     });
@@ -452,7 +456,7 @@ int init_state(grmhd* h) {
   if (rc) return rc;
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 0);
   CKL("k_reset_state");
-  k_post<true><<<grd3(g.nx + 2 * G + 1, g.ny + 2 * G + 1, g.nz + 2 * G + 1), blk3(), 0, h->s>>>(
+  k_post<true><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
       h->base, nullptr, g, h->E, h->dst, 1);
   CKL("k_post");
   return GRMHD_OK;

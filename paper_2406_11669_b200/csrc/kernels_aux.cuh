@@ -218,9 +218,9 @@ __device__ __forceinline__ void block_max3_atomic(double m0, double m1, double m
                                                   unsigned long long* acc) {
   __shared__ double sm[3][32];
   const int lane = threadIdx.x & 31;
-  const int tid = threadIdx.x + blockDim.x * threadIdx.y;
+  const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
   const int warp = tid >> 5;
-  const int nw = (blockDim.x * blockDim.y + 31) >> 5;
+  const int nw = (blockDim.x * blockDim.y * blockDim.z + 31) >> 5;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
     m0 = fmax(m0, __shfl_xor_sync(0xffffffffu, m0, o));
@@ -399,14 +399,25 @@ __device__ __forceinline__ void cell_sources(const double* __restrict__ base, co
 //   R9   stores alpha sqrt(gamma) S of those primitives for the next k_update,
 //   R16  accumulates the max characteristic speeds when want_speed.
 // One thread per padded index (i,j,k) in [-G, n+G].
+#ifndef KP_BY
+#define KP_BY 4
+#endif
+#ifndef KP_BZ
+#define KP_BZ 1
+#endif
+constexpr int KP_THREADS = 32 * KP_BY * KP_BZ;
+#ifndef KP_MINB
+#define KP_MINB 5
+#endif
 template <bool INIT>
-__global__ void __launch_bounds__(128, 4)
+__global__ void __launch_bounds__(KP_THREADS, KP_MINB)
 k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
        DevState* __restrict__ st, int want_speed) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x - G;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y - G;
-  const int k = blockIdx.z - G;
-  const bool inpad = i <= g.nx + G && j <= g.ny + G;
+  const int i = blockIdx.x * 32 + threadIdx.x - G;
+  const int j = blockIdx.y * KP_BY + threadIdx.y - G;
+  const int kraw = blockIdx.z * KP_BZ + threadIdx.z - G;
+  const int k = min(kraw, g.nz + G);
+  const bool inpad = i <= g.nx + G && j <= g.ny + G && kraw <= g.nz + G;
   const int c = (int)g.at(min(i, g.nx + G), min(j, g.ny + G), k);
   const bool ix = i < g.nx + G, jy = j < g.ny + G, kz = k < g.nz + G;
   double Bx = 0.0, By = 0.0, Bz = 0.0;
@@ -438,7 +449,7 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
       fld(base, g, F_BC + 2)[c] = Bz;
     }
   }
-  const bool in = i >= 0 && i < g.nx && j >= 0 && j < g.ny && k >= 0 && k < g.nz;
+  const bool in = inpad && i >= 0 && i < g.nx && j >= 0 && j < g.ny && k >= 0 && k < g.nz;
   double s[3] = {0.0, 0.0, 0.0};
   int bits = 0, iters = 0;
   if (in) {
@@ -481,7 +492,7 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
       const int np = __popc(__ballot_sync(0xffffffffu, (bits & 4) != 0));
       const int na = __popc(__ballot_sync(0xffffffffu, (bits & 1) != 0));
       const int nw = __popc(__ballot_sync(0xffffffffu, (bits & 8) != 0));
-      if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) {
+      if (threadIdx.x == 0) {
         if (nf) atomicAdd((unsigned long long*)&st->c2p_fail, (unsigned long long)nf);
         if (np) atomicAdd((unsigned long long*)&st->p_fix, (unsigned long long)np);
         if (na) atomicAdd((unsigned long long*)&st->atmo, (unsigned long long)na);
@@ -491,7 +502,7 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
     int mi = iters;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) mi = max(mi, __shfl_xor_sync(0xffffffffu, mi, o));
-    if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0 && mi > 0)
+    if (threadIdx.x == 0 && mi > 0)
       atomicMax((long long*)&st->c2p_maxiter, (long long)mi);
   }
   if (want_speed) block_max3_atomic(s[0], s[1], s[2], st->ms_acc);

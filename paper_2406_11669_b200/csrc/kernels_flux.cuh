@@ -101,55 +101,54 @@ __device__ __forceinline__ void rk_apply(double* __restrict__ base, const Geom& 
   }
 }
 
-// One thread per index (i,j,k) in [0,nx]x[0,ny]x[0,nz]: the cell's hydro update (if it is
-// an interior cell) and the three edges attached to it in the lower convention.  The
-// sources alpha sqrt(gamma) S were stored by k_post (kernels_aux.cuh) when the primitives
-// they depend on were recovered, so this kernel only streams: fluxes, sources, Y, Y0.
-__global__ void __launch_bounds__(256, 3)
+// One thread per evolved value: blockIdx.z = 8 k + r, r = row of Y (0-4 hydro rows of cell
+// (i,j,k); 5-7 the edges A_x, A_y, A_z attached to index (i,j,k) in the lower convention).
+// Each thread streams at most 6 flux values, one source, Y and Y0 -- all accesses are
+// coalesced along x, the row is uniform per block (no divergence) and the register need is
+// small enough for full occupancy.  The sources alpha sqrt(gamma) S were stored by k_post
+// (kernels_aux.cuh) when the primitives they depend on were recovered.
+__global__ void __launch_bounds__(256)
 k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
+  const int k = blockIdx.z >> 3;
+  const int r = blockIdx.z & 7;
   if (i > g.nx || j > g.ny) return;
   const long long c = g.at(i, j, k);
   const double h = st->dt;
   const long long sy = g.sy, sz = g.sz;
-
-  if (i < g.nx && j < g.ny && k < g.nz) {
+  double rhs;
+  if (r < 5) {
+    if (i >= g.nx || j >= g.ny || k >= g.nz) return;
     // R8: L(U~) = -sum_d (F~_{i+1/2} - F~_{i-1/2})/dx_d + alpha sqrt(gamma) S, eq. (17)
-#pragma unroll
-    for (int r = 0; r < 5; r++) {
-      const double* Fx = fld(base, g, F_FX + r);
-      const double* Fy = fld(base, g, F_FY + r);
-      const double* Fz = fld(base, g, F_FZ + r);
-      double div = (Fx[c + 1] - Fx[c]) * g.idx[0];
-      div += (Fy[c + sy] - Fy[c]) * g.idx[1];
-      div += (Fz[c + sz] - Fz[c]) * g.idx[2];
-      const double src = r == 0 ? 0.0 : fld(base, g, F_SRC + r - 1)[c];  // S_D = 0
-      rk_apply(base, g, r, c, -div + src, h, rk);
-    }
+    const double* Fx = fld(base, g, F_FX + r);
+    const double* Fy = fld(base, g, F_FY + r);
+    const double* Fz = fld(base, g, F_FZ + r);
+    double div = (Fx[c + 1] - Fx[c]) * g.idx[0];
+    div += (Fy[c + sy] - Fy[c]) * g.idx[1];
+    div += (Fz[c + sz] - Fz[c]) * g.idx[2];
+    const double src = r == 0 ? 0.0 : fld(base, g, F_SRC + r - 1)[c];  // S_D = 0
+    rhs = -div + src;
+  } else if (r == 5) {
+    // R10 (flux-CT, G13/G14) and R11 (d_t A_i = -E_i).  Stored B rows:
+    // FX+5 = F~x(B~y), FX+6 = F~x(B~z); FY+5 = F~y(B~z), FY+6 = F~y(B~x);
+    // FZ+5 = F~z(B~x), FZ+6 = F~z(B~y).
+    if (i >= g.nx) return;  // E_x at (i, j-1/2, k-1/2)
+    const double* FyBz = fld(base, g, F_FY + 5);
+    const double* FzBy = fld(base, g, F_FZ + 6);
+    rhs = -0.25 * (-FyBz[c - sz] - FyBz[c] + FzBy[c - sy] + FzBy[c]);
+  } else if (r == 6) {
+    if (j >= g.ny) return;  // E_y at (i-1/2, j, k-1/2)
+    const double* FzBx = fld(base, g, F_FZ + 5);
+    const double* FxBz = fld(base, g, F_FX + 6);
+    rhs = -0.25 * (-FzBx[c - 1] - FzBx[c] + FxBz[c - sz] + FxBz[c]);
+  } else {
+    if (k >= g.nz) return;  // E_z at (i-1/2, j-1/2, k)
+    const double* FxBy = fld(base, g, F_FX + 5);
+    const double* FyBx = fld(base, g, F_FY + 6);
+    rhs = -0.25 * (-FxBy[c - sy] - FxBy[c] + FyBx[c - 1] + FyBx[c]);
   }
-  // R10 (flux-CT, G13/G14) and R11 (d_t A_i = -E_i).  Stored B rows:
-  // FX+5 = F~x(B~y), FX+6 = F~x(B~z); FY+5 = F~y(B~z), FY+6 = F~y(B~x);
-  // FZ+5 = F~z(B~x), FZ+6 = F~z(B~y).
-  const double* FxBy = fld(base, g, F_FX + 5);
-  const double* FxBz = fld(base, g, F_FX + 6);
-  const double* FyBz = fld(base, g, F_FY + 5);
-  const double* FyBx = fld(base, g, F_FY + 6);
-  const double* FzBx = fld(base, g, F_FZ + 5);
-  const double* FzBy = fld(base, g, F_FZ + 6);
-  if (i < g.nx) {  // E_x at (i, j-1/2, k-1/2)
-    const double Ex = 0.25 * (-FyBz[c - sz] - FyBz[c] + FzBy[c - sy] + FzBy[c]);
-    rk_apply(base, g, 5, c, -Ex, h, rk);
-  }
-  if (j < g.ny) {  // E_y at (i-1/2, j, k-1/2)
-    const double Ey = 0.25 * (-FzBx[c - 1] - FzBx[c] + FxBz[c - sz] + FxBz[c]);
-    rk_apply(base, g, 6, c, -Ey, h, rk);
-  }
-  if (k < g.nz) {  // E_z at (i-1/2, j-1/2, k)
-    const double Ez = 0.25 * (-FxBy[c - sy] - FxBy[c] + FyBx[c - 1] + FyBx[c]);
-    rk_apply(base, g, 7, c, -Ez, h, rk);
-  }
+  rk_apply(base, g, r, c, rhs, h, rk);
 }
 
 }  // namespace gk
