@@ -189,9 +189,11 @@ ALG_BYTES = {  # algorithmic bytes per interior cell and launch (DESIGN.md "Roof
     "flux_z": FLUX_BYTES_PER_CELL_DIR,
     # update: fluxes 15 + 6, sources 4, Y 8, Y0 8 read; Y 8 written
     "update": (21 + 4 + 8 + 8 + 8) * 8,
-    # fused post-update kernel (curl A, con2prim, sources, max speed): A 3, B~0 3, metric 16,
-    # U~ 5 read; B~ 3, B_c 3, P 5, sources 4 written
-    "con2prim": (3 + 3 + 16 + 5 + 3 + 3 + 5 + 4) * 8,
+    # fused post-update kernel (curl A, con2prim, max speed): A 3, B~0 3, alpha/beta/gamma 10,
+    # U~ 5 read; B~ 3, B_c 3, P 5 written
+    "con2prim": (3 + 3 + 10 + 5 + 3 + 3 + 5) * 8,
+    # sources: P 5, B_c 3, metric 16 read; 4 written
+    "sources": (5 + 3 + 16 + 4) * 8,
 }
 
 

@@ -146,10 +146,11 @@ int grmhd_get_stats(grmhd* h, grmhd_stats* out);
 
 /* Device time per kernel group since "kernel_timing" was switched on (measurement aid for
  * the roofline report; synchronises).  Groups: 0 flux-x, 1 flux-y, 2 flux-z (A3+A4),
- * 3 divergence+sources+flux-CT+RK update (A5-A7), 4 A_i ghost fill + B from A (A1,A6),
- * 5 con2prim (A2, +A8 on the last stage), 6 primitive ghost fill (A1), 7 dt scalars.
+ * 3 divergence + flux-CT + RK update (A5-A7), 4 A_i ghost fill (A1),
+ * 5 B from A + con2prim (A6, A2, +A8 on the last stage), 6 primitive ghost fill (A1),
+ * 7 dt scalars, 8 metric source terms (A5, eq. 19).
  * ms[q] = summed milliseconds, launches[q] = number of timed brackets. */
-#define GRMHD_NKGROUPS 8
+#define GRMHD_NKGROUPS 9
 int grmhd_get_kernel_times(grmhd* h, double ms[GRMHD_NKGROUPS],
                            long long launches[GRMHD_NKGROUPS]);
 

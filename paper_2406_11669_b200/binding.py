@@ -247,12 +247,12 @@ class Solver:
         return d
 
     KERNEL_GROUPS = ("flux_x", "flux_y", "flux_z", "update", "bfield", "con2prim", "ghost_prims",
-                     "dt")
+                     "dt", "sources")
 
     def kernel_times(self) -> dict:
         """{group: (summed ms, brackets)} since set_option("kernel_timing", 1)."""
-        ms = (C.c_double * 8)()
-        cnt = (C.c_longlong * 8)()
+        ms = (C.c_double * 9)()
+        cnt = (C.c_longlong * 9)()
         self._chk(lib().grmhd_get_kernel_times(self.h, ms, cnt), "grmhd_get_kernel_times")
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_GROUPS)}
 

@@ -73,7 +73,7 @@ int cuda_fail(grmhd* h, cudaError_t e, const char* where) {
   } while (0)
 
 // ---- kernel-group timing -------------------------------------------------------------
-enum { KG_FLUX_X = 0, KG_FLUX_Y, KG_FLUX_Z, KG_UPDATE, KG_BFIELD, KG_C2P, KG_GHOST, KG_MISC };
+enum { KG_FLUX_X = 0, KG_FLUX_Y, KG_FLUX_Z, KG_UPDATE, KG_BFIELD, KG_C2P, KG_GHOST, KG_MISC, KG_SRC };
 
 int kt_flush(grmhd* h) {
   if (h->ev_used == 0) return GRMHD_OK;
@@ -181,6 +181,9 @@ dim3 grd_post(const Geom& g) {
   return dim3((g.nx + 2 * G + 1 + 31) / 32, (g.ny + 2 * G + 1 + KP_BY - 1) / KP_BY,
               (g.nz + 2 * G + 1 + KP_BZ - 1) / KP_BZ);
 }
+dim3 grd_src(const Geom& g) {
+  return dim3((g.nx + KS_BX - 1) / KS_BX, (g.ny + KS_BY - 1) / KS_BY, g.nz);
+}
 int grd1(long long n) {
   long long b = (n + 255) / 256;
   return (int)(b > 65535 * 16 ? 65535 * 16 : (b < 1 ? 1 : b));
@@ -269,6 +272,10 @@ int after_stage(grmhd* h, bool want_speed) {
         h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
     CKL("k_post");
   });
+  KT(KG_SRC, {
+    k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
+    CKL("k_src");
+  });
   KT(KG_GHOST, {
     rc = fill_ghosts(h, fill_prims());
     if (rc) return rc;
@@ -315,6 +322,9 @@ int launch_flux(grmhd* h, int apron) {
 }
 
 // ---- TMA-fed flux kernel (flux_tma.cuh) ---------------------------------------------------
+#ifndef FT_PROMO_X
+#define FT_PROMO_X CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -343,7 +353,9 @@ bool make_tensor_maps(grmhd* h) {
       CUresult r = ((EncodeTiledFn)fn)(w == 0 ? &h->tm_met[d] : &h->tm_bf[d],
                                        CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, h->base, dims, strides,
                                        box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                       CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                       CU_TENSOR_MAP_SWIZZLE_NONE,
+                                       d == 0 ? (CUtensorMapL2promotion)FT_PROMO_X
+                                              : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
       if (r != CUDA_SUCCESS) return false;
     }
@@ -459,6 +471,8 @@ int init_state(grmhd* h) {
   k_post<true><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
       h->base, nullptr, g, h->E, h->dst, 1);
   CKL("k_post");
+  k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
+  CKL("k_src");
   return GRMHD_OK;
 }
 

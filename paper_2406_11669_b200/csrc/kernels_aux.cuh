@@ -478,10 +478,6 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
       }
     }
     const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
-    double S[4];
-    cell_sources(base, g, c, P, M, sg, E, S);
-#pragma unroll
-    for (int r = 0; r < 4; r++) fld(base, g, F_SRC + r)[c] = S[r];
     if (want_speed) cell_speeds(P, M, E, s);
   }
   if (!INIT) {
@@ -506,6 +502,35 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
       atomicMax((long long*)&st->c2p_maxiter, (long long)mi);
   }
   if (want_speed) block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
+}
+
+// R9: alpha sqrt(gamma) S of the interior cells from the primitives k_post just stored, for
+// the next k_update.  Its own kernel: the 120 stencil loads of the metric derivatives want
+// L1 and registers that the Newton iteration of k_post would otherwise hold.
+#ifndef KS_MINB
+#define KS_MINB 4
+#endif
+#ifndef KS_BX
+#define KS_BX 32
+#endif
+#ifndef KS_BY
+#define KS_BY 4
+#endif
+__global__ void __launch_bounds__(KS_BX * KS_BY, KS_MINB)
+k_src(double* __restrict__ base, Geom g, Eos E) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z;
+  if (i >= g.nx || j >= g.ny) return;
+  const int c = (int)g.at(i, j, k);
+  const Met M = load_met(base, g, c);
+  const Prim P = load_prim(base, g, c);
+  const double det = det_gamma(M);
+  const double sg = det * ft_rsqrt(det);
+  double S[4];
+  cell_sources(base, g, c, P, M, sg, E, S);
+#pragma unroll
+  for (int r = 0; r < 4; r++) fld(base, g, F_SRC + r)[c] = S[r];
 }
 
 // ---------------------------------------------------------------------------------- dt
