@@ -359,7 +359,6 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
   FtMarch<RECON> mv[2];
   FtFlat fmch;
   double nxt[2][TC];        // cells of the next chunk (prefetched)
-  double pnx[TC], vnx[TC];  // flattening inputs of the chunk after the next
   // ---- prologue: state before cell f0-1, flattening of f0-1 and of chunk 0
 #pragma unroll
   for (int s = 0; s < 2; s++) {
@@ -378,10 +377,6 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
       const int cc = f0 + cl;
       sm.fl[0][cl][lane] = fmch.step(psrc[min(cc + 2, cmax) * sd], vsrc[min(cc + 1, cmax) * sd]);
     }
-    // inputs of the flattening of chunk 1 (cells f0+4 .. f0+7): p_{c+2}, v_{c+1}
-    load_cells(psrc, f0 + TC, pnx);
-#pragma unroll
-    for (int cl = 0; cl < TC; cl++) vnx[cl] = vsrc[min(f0 + TC + cl + 1, cmax) * sd];
   }
   __syncthreads();  // barrier init + fl0 / fl[0] visible
   {
@@ -402,9 +397,10 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
   if (D == 0) { clB = tid % TC; plB = tid / TC; }
   else { plB = lane; clB = warp; }
   const bool okB = g0 + plB < nt0;
-  const int pB = min(g0 + plB, nt0 - 1);
-  const int baseB = (int)(D == 0 ? g.at(0, pB, t1) : (D == 1 ? g.at(pB, 0, t1) : g.at(pB, t1, 0)));
-  double* const outp = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + baseB;
+  // output offset = block-uniform part + a term rebuilt from the thread index when needed
+  // (nothing to keep in a register across the loop)
+  const long long ublk = D == 0 ? g.at(0, g0, t1) : (D == 1 ? g.at(g0, 0, t1) : g.at(g0, t1, 0));
+  double* const outb = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + ublk;
   const size_t NPA = (size_t)g.NPA;
   // ring offsets of the thread: layer j = clB + k of the 8 resident ones
   constexpr int MF = TC * 32;  // doubles per field in a slot
@@ -424,6 +420,14 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
 #pragma unroll
     for (int s = 0; s < 2; s++)
       if (s < nslot && more) load_cells(qsrc[s], F + TC, nxt[s]);
+    // warp 3 (one variable): inputs p_{c+2}, v_{c+1} of the flattening of the next chunk's
+    // cells, in flight while its variable is reconstructed
+    double pc[TC], vc[TC];
+    if (RECON == 2 && warp == 3 && more) {
+      load_cells(psrc, F + TC, pc);
+#pragma unroll
+      for (int cl = 0; cl < TC; cl++) vc[cl] = vsrc[min(F + TC + cl + 1, cmax) * sd];
+    }
 #pragma unroll
     for (int s = 0; s < 2; s++) {
       if (s < nslot) {
@@ -440,14 +444,6 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
       }
     }
     if (RECON == 2 && warp == 3 && more) {
-      double pc[TC], vc[TC];
-#pragma unroll
-      for (int cl = 0; cl < TC; cl++) { pc[cl] = pnx[cl]; vc[cl] = vnx[cl]; }
-      if (n + 2 < nchunk) {
-        load_cells(psrc, F + 2 * TC, pnx);
-#pragma unroll
-        for (int cl = 0; cl < TC; cl++) vnx[cl] = vsrc[min(F + 2 * TC + cl + 1, cmax) * sd];
-      }
 #pragma unroll
       for (int cl = 0; cl < TC; cl++) sm.fl[buf ^ 1][cl][lane] = fmch.step(pc[cl], vc[cl]);
     }
@@ -500,7 +496,8 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
       double out[7];
       ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
       if (okB && f >= 0 && f < f1) {
-        double* o = outp + f * sd;
+        const int pl = D == 0 ? tid / TC : (tid & 31);
+        double* o = outb + (D == 0 ? pl * (int)g.sy + f : pl + f * sd);
 #pragma unroll
         for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
       }
