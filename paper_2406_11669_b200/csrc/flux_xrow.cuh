@@ -1,0 +1,142 @@
+// flux_xrow.cuh -- A3 + A4 along x with the lanes of a warp ALONG x.
+//
+// x is the contiguous axis: a kernel that marches along x (flux_tma.cuh, D = 0) can only
+// touch 32 bytes of a row at a time, which HBM serves badly (ncu capture r1g: the prefetched
+// cells arrive late, DRAM reads 1.45x the algorithmic bytes).  Here a warp owns 32 consecutive
+// cells c0 .. c0+31 of one row (j, k); lane = cell.  Every load and store is a contiguous
+// 256-byte row segment.  The reconstruction recurrences run across lanes: the limited slope,
+// the interface value and the parabola of a cell are computed once, by the cell's lane, and
+// handed to the neighbour with warp shuffles (R5/G8: slope of c+1 from the lane above,
+// interface c-1/2 and q^+_{c-1} from the lane below).  The lane of cell c then solves the
+// Riemann problem of face c-1/2.  The 3 lowest and 2 highest lanes have incomplete stencils:
+// a warp yields 27 faces; consecutive warps overlap by 5 cells.  No shared memory, no block
+// barrier, nothing carried from one row segment to the next.
+#pragma once
+#include "flux_tma.cuh"
+
+namespace gk {
+
+constexpr int FX_THREADS = 128;
+constexpr int FX_VALID = 27;  // faces per warp: lanes 3 .. 29
+
+__device__ __forceinline__ double fx_up(double v, int d) {
+  return __shfl_up_sync(0xffffffffu, v, d);
+}
+__device__ __forceinline__ double fx_dn(double v, int d) {
+  return __shfl_down_sync(0xffffffffu, v, d);
+}
+
+// q^-_c (right state of face c-1/2) and q^+_c of the lane's cell; qm1, qp1 = neighbours
+template <int RECON>
+__device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, double f, bool anyf,
+                                         double& qm, double& qp) {
+  const double dl = q - qm1, dr = qp1 - q;
+  if (RECON == 0) {  // G7
+    const double m = fabs(dl) < fabs(dr) ? dl : dr;
+    const double s = dl * dr > 0.0 ? m : 0.0;
+    qm = fma(-0.5, s, q);
+    qp = fma(0.5, s, q);
+  } else {  // G8(a)-(d), same arithmetic as FtMarch::step
+    const double dm = ft_slope(dl, dr);
+    const double dmp = fx_dn(dm, 1);                             // slope of cell c+1
+    const double ir = 0.5 * (q + qp1) - (dmp - dm) * (1.0 / 6.0);  // interface c + 1/2
+    const double il = fx_up(ir, 1);                              // interface c - 1/2
+    qm = il; qp = ir;
+    if (RECON == 2 && anyf) {
+      const double qpf = f * q + (1.0 - f) * qp;
+      const double qmf = f * q + (1.0 - f) * qm;
+      qp = f != 0.0 ? qpf : qp;
+      qm = f != 0.0 ? qmf : qm;
+    }
+    const double a = qp - q, b = q - qm;
+    const double aa = fabs(a), ab = fabs(b);
+    const bool flat = a * b <= 0.0;
+    const bool fixm = ab > 2.0 * aa;
+    const bool fixp = aa > 2.0 * ab;
+    const double qm2 = fma(-2.0, a, q);
+    const double qp2 = fma(2.0, b, q);
+    qm = ft_sel(flat, q, ft_sel(fixm, qm2, qm));
+    qp = ft_sel(flat, q, ft_sel(fixp, qp2, qp));
+  }
+}
+
+// grid: one warp per (row, segment) item; item = row * nsx + seg, row = (k+1)*(ny+2) + (j+1)
+template <int RECON>
+__global__ void __launch_bounds__(FX_THREADS, 3)
+k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems) {
+  const int lane = threadIdx.x & 31;
+  const long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
+  if (item >= nitems) return;  // warp uniform
+  const int seg = (int)(item % nsx);
+  const int row = (int)(item / nsx);
+  const int j = row % (g.ny + 2) - 1;
+  const int k = row / (g.ny + 2) - 1;
+  const int c = seg * FX_VALID - 3 + lane;  // this lane's cell; its face is c - 1/2
+  const int cc = min(c, g.nx + G - 1);      // lanes past the last ghost cell reuse it
+  const int idx = (int)g.at(cc, j, k);
+
+  // ---- cell data of the lane: rho, v^x, v^y, v^z, p, B^y, B^z
+  double q[FM_NV];
+#pragma unroll
+  for (int v = 0; v < FM_NV; v++) q[v] = fld(base, g, fm_var_field(0, v))[idx];
+  const double bfx = fld(base, g, F_BF + 0)[idx];
+  // ---- face metric (R4): 4-point Lagrange along x
+  Met M;
+  {
+    double mq[FT_NMET];
+#pragma unroll
+    for (int v = 0; v < FT_NMET; v++) {
+      const double* m = fld(base, g, F_MET + v) + idx;
+      mq[v] = (-m[-2] + 9.0 * m[-1] + 9.0 * m[0] - m[1]) * 0.0625;
+    }
+    M.a = mq[0]; M.bx = mq[1]; M.by = mq[2]; M.bz = mq[3];
+    M.gxx = mq[4]; M.gxy = mq[5]; M.gxz = mq[6]; M.gyy = mq[7]; M.gyz = mq[8]; M.gzz = mq[9];
+  }
+  // ---- neighbours across lanes
+  double qm1[FM_NV], qp1[FM_NV];
+#pragma unroll
+  for (int v = 0; v < FM_NV; v++) { qm1[v] = fx_up(q[v], 1); qp1[v] = fx_dn(q[v], 1); }
+  // G8(c): flattening coefficient of the lane's cell from p_{c-2..c+2}, v^x_{c-1}, v^x_{c+1}
+  double f = 0.0;
+  bool anyf = false;
+  if (RECON == 2) {
+    const double pm2 = fx_up(q[4], 2), pp2 = fx_dn(q[4], 2);
+    const double dp1 = qp1[4] - qm1[4];
+    const double dp2 = pp2 - pm2;
+    const bool on = fabs(dp1) > 0.33 * ft_min(qp1[4], qm1[4]) && qm1[1] > qp1[1];
+    const bool z = dp2 == 0.0;
+    const double r = ft_rcp(z ? 1.0 : dp2);
+    double ff = 10.0 * fma(dp1, r, -0.75);
+    ff = ft_min(1.0, ft_max(0.0, ff));
+    ff = z ? 1.0 : ff;
+    f = on ? ff : 0.0;
+    anyf = __any_sync(0xffffffffu, f != 0.0);
+  }
+  double qL[FM_NV], qR[FM_NV];
+#pragma unroll
+  for (int v = 0; v < FM_NV; v++) {
+    double qm, qp;
+    fx_recon<RECON>(q[v], qm1[v], qp1[v], f, anyf, qm, qp);
+    qL[v] = fx_up(qp, 1);  // q^+ of cell c-1
+    qR[v] = qm;
+  }
+  // ---- Riemann problem of face c - 1/2 (R7)
+  const double det = det_gamma(M);
+  const double isg = ft_rsqrt(det);
+  const double sgf = det * isg;
+  const double gdd = inv_gamma_dd<0>(M, isg * isg);
+  const double Bn = bfx * isg;  // G6
+  double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR;
+  ft_side<0>(qL[0], qL[1], qL[2], qL[3], qL[4], Bn, qL[5], qL[6], M, gdd, E, UL, GL, lmL, lpL);
+  ft_side<0>(qR[0], qR[1], qR[2], qR[3], qR[4], Bn, qR[5], qR[6], M, gdd, E, UR, GR, lmR, lpR);
+  double out[7];
+  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
+  if (lane >= 3 && lane < 3 + FX_VALID && c <= g.nx) {
+    double* o = fld(base, g, F_FX) + idx;
+    const size_t NPA = (size_t)g.NPA;
+#pragma unroll
+    for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
+  }
+}
+
+}  // namespace gk

@@ -13,6 +13,7 @@
 #include "kernels_flux.cuh"
 #include "flux_march.cuh"
 #include "flux_tma.cuh"
+#include "flux_xrow.cuh"
 #include "kernels_batch.cuh"
 
 using namespace gk;
@@ -36,6 +37,7 @@ struct grmhd {
   int ft_conc[9] = {0};  // ... of the TMA-fed instantiations
   CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][.] of the ring stages, per direction
   bool tma_ok = false;
+  int xrow = 1;          // x fluxes: 1 k_flux_xrow (lanes along x), 0 as y and z
   int flux_impl = 1;     // 1: k_flux_tma (+ k_flux_march on the apron columns), 0: k_flux_march
   char err[256] = {0};
   // optional per-kernel-group timing ("kernel_timing" option): CUDA events on the stream
@@ -402,12 +404,27 @@ int launch_flux_tma(grmhd* h) {
   return launch_flux<D, RECON>(h, 1);  // the two apron columns along t0
 }
 
+// x fluxes with the lanes along x (flux_xrow.cuh): one warp per 27 faces of a row
+template <int RECON>
+int launch_flux_xrow(grmhd* h) {
+  const Geom& g = h->g;
+  const int nsx = (g.nx + 1 + FX_VALID - 1) / FX_VALID;
+  const long long nitems = (long long)nsx * (g.ny + 2) * (g.nz + 2);
+  const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
+  k_flux_xrow<RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsx, nitems);
+  h->launches++;
+  return GRMHD_OK;
+}
+
 template <int D>
 int launch_flux_d(grmhd* h) {
   const int recon = h->o.recon == 0 ? 0 : (h->o.ppm_flatten ? 2 : 1);
   const int nt0 = D == 0 ? h->g.ny : h->g.nx;
   int rc;
-  if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
+  if (D == 0 && h->flux_impl == 1 && h->xrow)
+    rc = recon == 0 ? launch_flux_xrow<0>(h)
+                    : (recon == 1 ? launch_flux_xrow<1>(h) : launch_flux_xrow<2>(h));
+  else if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
     rc = recon == 0 ? launch_flux_tma<D, 0>(h)
                     : (recon == 1 ? launch_flux_tma<D, 1>(h) : launch_flux_tma<D, 2>(h));
   else
@@ -694,6 +711,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "flux_kernel") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
     h->flux_impl = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "flux_x_rows") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_x_rows is 0 or 1");
+    h->xrow = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "kernel_timing") == 0) {
