@@ -43,9 +43,11 @@ def _assert_cons(Ug, Ur, tol, what):
     return errs
 
 
-def _one_step_case(w, nsteps=1, tol=TOL1):
+def _one_step_case(w, nsteps=1, tol=TOL1, gpu_options=None):
     r = make_ref(w)
     g = make_gpu(w)
+    for key, val in (gpu_options or {}).items():
+        g.set_option(key, val)
     # state right after set_*: conserved variables, primitives incl. ghosts, stats
     _assert_cons(to_np(g.get_cons()), r.get_cons(), 1e-13, w.name + " init")
     sg, sr = g.stats(), r.stats()
@@ -156,6 +158,83 @@ def test_tiny_and_degenerate_blocks():
     _one_step_case(wl.alfven_wave(1, 16, 1, axis=1), nsteps=3)
     _one_step_case(wl.alfven_wave(1, 1, 16, axis=2), nsteps=3)
     _one_step_case(wl.balsara1(8, 2, 2), nsteps=2)
+
+
+def test_every_flux_kernel_is_covered():
+    """The three implementations of A3+A4 give the oracle's result: k_flux_xrow + k_flux_tma
+    (default), k_flux_tma for x as well, and the marching kernel k_flux_march everywhere."""
+    for opts in ({"flux_x_rows": 0.0}, {"flux_kernel": 0.0}):
+        _one_step_case(wl.kerr_blob(40), gpu_options=opts)
+        _one_step_case(wl.blast(44), gpu_options=opts)
+        w = wl.c2p_stress(36)
+        w2 = wl.Workload(**{**w.__dict__, "opts": {**w.opts, "recon": 0, "rk": 2},
+                            "name": w.name + "_minmod"})
+        _one_step_case(w2, gpu_options=opts)
+
+
+# ------------------------------------------------- full BASELINE sizes, bench configuration
+def test_config2_blast_full_size_one_step():
+    _one_step_case(wl.make(1))            # 128^3, the launch configuration bench.py times
+
+
+def test_config3_kerr_full_size_one_step():
+    _one_step_case(wl.make(2))            # 256^3 Kerr-Schild: the bench workload
+
+
+def test_config4_c2p_stress_full_size_one_step():
+    """256^3 generic metric, W up to 10, sigma up to 10.  One RK3 step of this stress field
+    drives a handful of cells to the edge of the con2prim domain (measured: 1 cell of 16.8 M,
+    p/rho = 10, W = 10 after the step), where the recovery amplifies rounding differences of
+    the two fp64 implementations by ~1e5.  So: 1e-11 on every field once
+    at most 1e-6 of the cells are set aside, and 1e-10 on all cells."""
+    w = wl.make(3)
+    r, g = make_ref(w), make_gpu(w)
+    r.step(1, w.cfl)
+    g.step(1, w.cfl)
+    Ug, Ur = to_np(g.get_cons()), r.get_cons()
+    _assert_cons(Ug, Ur, 1e-10, w.name + " all cells")
+    ncell = w.nx * w.ny * w.nz
+    for grp in ((0,), (1, 2, 3), (4,), (5, 6, 7)):
+        scale = max(np.abs(interior(Ur[q])).max() for q in grp)
+        for q in grp:
+            nbad = int((np.abs(interior(Ug[q]) - interior(Ur[q])) > TOL1 * scale).sum())
+            REPORT.append({"case": f"{w.name} field {q}: cells above 1e-11", "tol": 1e-6 * ncell,
+                           "max": nbad})
+            assert nbad <= 1e-6 * ncell, (q, nbad)
+    sg, sr = g.stats(), r.stats()
+    for k in ("c2p_fail", "atmo", "w_cap"):
+        assert sg[k] == sr[k], (k, sg[k], sr[k])
+    g.close()
+
+
+def test_config5_bns_quarter_size_one_step():
+    """Config 5 at 128^3 (the oracle's 512^3 state would need ~80 GB of host memory); the
+    512^3 launch configuration itself is exercised by test_config5_full_size_properties."""
+    _one_step_case(wl.bns_like(128))
+
+
+@pytest.mark.skipif(__import__("os").environ.get("GRMHD_TEST_512") != "1",
+                    reason="512^3 (88 GB workspace, ~30 GB of host arrays): set GRMHD_TEST_512=1")
+def test_config5_full_size_properties():
+    """512^3 RK4: properties that hold at any size -- finite state, no con2prim failure, the
+    densitised rest mass sum(sqrt(gamma) D) conserved to round-off on the periodic block."""
+    import torch
+    w = wl.make(4)
+    g = make_gpu(w)
+    I = (slice(3, -3),) * 3
+    # conformally flat metric of the workload: sqrt(gamma) = (gxx gyy gzz)^(1/2)
+    sg = torch.from_numpy(np.sqrt(w.metric[4][I] * w.metric[7][I] * w.metric[9][I])).cuda()
+    m0 = float((g.get_cons()[0][I].double() * sg).sum())
+    g.step(1, w.cfl)
+    st = g.stats()
+    assert st["rc"] == 0 and st["c2p_fail"] == 0 and np.isfinite(st["dt"]) and st["dt"] > 0
+    U = g.get_cons()
+    for u in U:
+        assert bool(torch.isfinite(u).all())
+    m1 = float((U[0][I].double() * sg).sum())
+    REPORT.append({"case": "config5 512^3 rest mass", "tol": 1e-12, "max": abs(m1 - m0) / m0})
+    assert abs(m1 - m0) <= 1e-12 * m0 or st["atmo"] > 0
+    g.close()
 
 
 # ------------------------------------------------------------------------- many steps
