@@ -18,6 +18,9 @@ namespace gk {
 
 constexpr int FX_THREADS = 128;
 constexpr int FX_VALID = 27;  // faces per warp: lanes 3 .. 29
+#ifndef FX_MINB
+#define FX_MINB 4
+#endif
 
 __device__ __forceinline__ double fx_up(double v, int d) {
   return __shfl_up_sync(0xffffffffu, v, d);
@@ -62,11 +65,13 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
 
 // grid: one warp per (row, segment) item; item = row * nsx + seg, row = (k+1)*(ny+2) + (j+1)
 template <int RECON>
-__global__ void __launch_bounds__(FX_THREADS, 3)
+__global__ void __launch_bounds__(FX_THREADS, FX_MINB)
 k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems) {
   const int lane = threadIdx.x & 31;
-  const long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
-  if (item >= nitems) return;  // warp uniform
+  const long long nwarp = (long long)gridDim.x * (FX_THREADS / 32);
+  // grid-stride loop over the items (the launch gives every warp one item)
+  for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
+       item < nitems; item += nwarp) {
   const int seg = (int)(item % nsx);
   const int row = (int)(item / nsx);
   const int j = row % (g.ny + 2) - 1;
@@ -137,6 +142,7 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems)
 #pragma unroll
     for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
   }
+  }  // items
 }
 
 }  // namespace gk
