@@ -32,7 +32,7 @@ FLUX_BYTES_PER_CELL_DIR = 26 * 8
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=2,
                     help="index into BASELINE.json configs (0..4); default 2 = 256^3 Kerr-Schild")

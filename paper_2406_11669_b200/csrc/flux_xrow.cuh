@@ -63,36 +63,48 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
   }
 }
 
-// grid: one warp per (row, segment) item; item = row * nsx + seg, row = (k+1)*(ny+2) + (j+1)
-template <int RECON>
+// grid: one warp per (pencil, segment) item.
+// D = 0: every row of the block incl. the flux-CT apron: item = row * nsd + seg,
+//        row = (k+1)*(ny+2) + (j+1).
+// D = 1, 2: only the two apron columns x = -1 and x = nx that the 32-wide groups of
+//        k_flux_tma leave out (lanes then run along y or z with a stride: uncoalesced, but
+//        it is 2 columns): item = ((t1+1) * 2 + col) * nsd + seg.
+template <int D, int RECON>
 __global__ void __launch_bounds__(FX_THREADS, FX_MINB)
-k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems) {
+k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems) {
   const int lane = threadIdx.x & 31;
   const long long nwarp = (long long)gridDim.x * (FX_THREADS / 32);
+  const int nD = g.n(D);
+  const int sd = D == 0 ? 1 : (D == 1 ? (int)g.sy : (int)g.sz);
   // grid-stride loop over the items (the launch gives every warp one item)
   for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
        item < nitems; item += nwarp) {
-  const int seg = (int)(item % nsx);
-  const int row = (int)(item / nsx);
-  const int j = row % (g.ny + 2) - 1;
-  const int k = row / (g.ny + 2) - 1;
-  const int c = seg * FX_VALID - 3 + lane;  // this lane's cell; its face is c - 1/2
-  const int cc = min(c, g.nx + G - 1);      // lanes past the last ghost cell reuse it
-  const int idx = (int)g.at(cc, j, k);
+  const int seg = (int)(item % nsd);
+  const int row = (int)(item / nsd);
+  const int c = seg * FX_VALID - 3 + lane;  // this lane's cell along D; its face is c - 1/2
+  const int cc = min(c, nD + G - 1);        // lanes past the last ghost cell reuse it
+  int idx;
+  if (D == 0) {
+    idx = (int)g.at(cc, row % (g.ny + 2) - 1, row / (g.ny + 2) - 1);
+  } else {
+    const int xc = (row & 1) ? g.nx : -1;
+    const int t1 = (row >> 1) - 1;
+    idx = (int)(D == 1 ? g.at(xc, cc, t1) : g.at(xc, t1, cc));
+  }
 
   // ---- cell data of the lane: rho, v^x, v^y, v^z, p, B^y, B^z
   double q[FM_NV];
 #pragma unroll
-  for (int v = 0; v < FM_NV; v++) q[v] = fld(base, g, fm_var_field(0, v))[idx];
-  const double bfx = fld(base, g, F_BF + 0)[idx];
-  // ---- face metric (R4): 4-point Lagrange along x
+  for (int v = 0; v < FM_NV; v++) q[v] = fld(base, g, fm_var_field(D, v))[idx];
+  const double bfx = fld(base, g, F_BF + D)[idx];
+  // ---- face metric (R4): 4-point Lagrange along D
   Met M;
   {
     double mq[FT_NMET];
 #pragma unroll
     for (int v = 0; v < FT_NMET; v++) {
       const double* m = fld(base, g, F_MET + v) + idx;
-      mq[v] = (-m[-2] + 9.0 * m[-1] + 9.0 * m[0] - m[1]) * 0.0625;
+      mq[v] = (-m[-2 * sd] + 9.0 * m[-sd] + 9.0 * m[0] - m[sd]) * 0.0625;
     }
     M.a = mq[0]; M.bx = mq[1]; M.by = mq[2]; M.bz = mq[3];
     M.gxx = mq[4]; M.gxy = mq[5]; M.gxz = mq[6]; M.gyy = mq[7]; M.gyz = mq[8]; M.gzz = mq[9];
@@ -101,14 +113,14 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems)
   double qm1[FM_NV], qp1[FM_NV];
 #pragma unroll
   for (int v = 0; v < FM_NV; v++) { qm1[v] = fx_up(q[v], 1); qp1[v] = fx_dn(q[v], 1); }
-  // G8(c): flattening coefficient of the lane's cell from p_{c-2..c+2}, v^x_{c-1}, v^x_{c+1}
+  // G8(c): flattening coefficient of the lane's cell from p_{c-2..c+2}, v^D_{c-1}, v^D_{c+1}
   double f = 0.0;
   bool anyf = false;
   if (RECON == 2) {
     const double pm2 = fx_up(q[4], 2), pp2 = fx_dn(q[4], 2);
     const double dp1 = qp1[4] - qm1[4];
     const double dp2 = pp2 - pm2;
-    const bool on = fabs(dp1) > 0.33 * ft_min(qp1[4], qm1[4]) && qm1[1] > qp1[1];
+    const bool on = fabs(dp1) > 0.33 * ft_min(qp1[4], qm1[4]) && qm1[1 + D] > qp1[1 + D];
     const bool z = dp2 == 0.0;
     const double r = ft_rcp(z ? 1.0 : dp2);
     double ff = 10.0 * fma(dp1, r, -0.75);
@@ -129,15 +141,20 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsx, long long nitems)
   const double det = det_gamma(M);
   const double isg = ft_rsqrt(det);
   const double sgf = det * isg;
-  const double gdd = inv_gamma_dd<0>(M, isg * isg);
+  const double gdd = inv_gamma_dd<D>(M, isg * isg);
   const double Bn = bfx * isg;  // G6
   double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR;
-  ft_side<0>(qL[0], qL[1], qL[2], qL[3], qL[4], Bn, qL[5], qL[6], M, gdd, E, UL, GL, lmL, lpL);
-  ft_side<0>(qR[0], qR[1], qR[2], qR[3], qR[4], Bn, qR[5], qR[6], M, gdd, E, UR, GR, lmR, lpR);
+  // slots 5, 6 hold B^{(D+1)%3}, B^{(D+2)%3}
+  ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
+             D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]), M,
+             gdd, E, UL, GL, lmL, lpL);
+  ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
+             D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]), M,
+             gdd, E, UR, GR, lmR, lpR);
   double out[7];
   ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
-  if (lane >= 3 && lane < 3 + FX_VALID && c <= g.nx) {
-    double* o = fld(base, g, F_FX) + idx;
+  if (lane >= 3 && lane < 3 + FX_VALID && c <= nD) {
+    double* o = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
     for (int r = 0; r < 7; r++) o[r * NPA] = out[r];

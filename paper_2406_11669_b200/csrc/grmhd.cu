@@ -323,6 +323,21 @@ int launch_flux(grmhd* h, int apron) {
   return GRMHD_OK;
 }
 
+// lanes along D (flux_xrow.cuh): one warp per 27 faces of a pencil.  D = 0: every row;
+// D = 1, 2: the two apron columns of k_flux_tma.
+template <int D, int RECON>
+int launch_flux_xrow(grmhd* h) {
+  const Geom& g = h->g;
+  const int nsd = (g.n(D) + 1 + FX_VALID - 1) / FX_VALID;
+  const long long npen = D == 0 ? (long long)(g.ny + 2) * (g.nz + 2)
+                                : 2LL * ((D == 2 ? g.ny : g.nz) + 2);
+  const long long nitems = npen * nsd;
+  const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
+  k_flux_xrow<D, RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd, nitems);
+  h->launches++;
+  return GRMHD_OK;
+}
+
 // ---- TMA-fed flux kernel (flux_tma.cuh) ---------------------------------------------------
 #ifndef FT_PROMO_X
 #define FT_PROMO_X CU_TENSOR_MAP_L2_PROMOTION_L2_256B
@@ -401,19 +416,9 @@ int launch_flux_tma(grmhd* h) {
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_tma");
-  return launch_flux<D, RECON>(h, 1);  // the two apron columns along t0
-}
-
-// x fluxes with the lanes along x (flux_xrow.cuh): one warp per 27 faces of a row
-template <int RECON>
-int launch_flux_xrow(grmhd* h) {
-  const Geom& g = h->g;
-  const int nsx = (g.nx + 1 + FX_VALID - 1) / FX_VALID;
-  const long long nitems = (long long)nsx * (g.ny + 2) * (g.nz + 2);
-  const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
-  k_flux_xrow<RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsx, nitems);
-  h->launches++;
-  return GRMHD_OK;
+  // the two apron columns along t0
+  if (D != 0 && h->xrow) return launch_flux_xrow<D, RECON>(h);
+  return launch_flux<D, RECON>(h, 1);
 }
 
 template <int D>
@@ -422,8 +427,8 @@ int launch_flux_d(grmhd* h) {
   const int nt0 = D == 0 ? h->g.ny : h->g.nx;
   int rc;
   if (D == 0 && h->flux_impl == 1 && h->xrow)
-    rc = recon == 0 ? launch_flux_xrow<0>(h)
-                    : (recon == 1 ? launch_flux_xrow<1>(h) : launch_flux_xrow<2>(h));
+    rc = recon == 0 ? launch_flux_xrow<0, 0>(h)
+                    : (recon == 1 ? launch_flux_xrow<0, 1>(h) : launch_flux_xrow<0, 2>(h));
   else if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
     rc = recon == 0 ? launch_flux_tma<D, 0>(h)
                     : (recon == 1 ? launch_flux_tma<D, 1>(h) : launch_flux_tma<D, 2>(h));
