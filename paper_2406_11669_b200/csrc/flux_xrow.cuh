@@ -97,13 +97,15 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems)
 #pragma unroll
   for (int v = 0; v < FM_NV; v++) q[v] = fld(base, g, fm_var_field(D, v))[idx];
   const double bfx = fld(base, g, F_BF + D)[idx];
-  // ---- face metric (R4): 4-point Lagrange along D
+  // ---- face metric (R4): 4-point Lagrange along D.  Lanes 0-2 have no face to solve: their
+  // stencil base is moved to cell -1 so that it stays inside the padded array.
+  const int idxm = idx + (max(cc, -1) - cc) * sd;
   Met M;
   {
     double mq[FT_NMET];
 #pragma unroll
     for (int v = 0; v < FT_NMET; v++) {
-      const double* m = fld(base, g, F_MET + v) + idx;
+      const double* m = fld(base, g, F_MET + v) + idxm;
       mq[v] = (-m[-2 * sd] + 9.0 * m[-sd] + 9.0 * m[0] - m[sd]) * 0.0625;
     }
     M.a = mq[0]; M.bx = mq[1]; M.by = mq[2]; M.bz = mq[3];
