@@ -308,6 +308,7 @@ def run_b200(args):
     roofline = {"kernel": "flux (reconstruct + Riemann, average of x/y/z launches)",
                 "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic_for(w.name),
+                "fp64_pipe_active_pct_ncu": traffic_for("_fp64_pipe_active_pct"),
                 "alg_bytes_per_launch": FLUX_BYTES_PER_CELL_DIR * w.ncells,
                 "ms_per_launch": flux_avg, "share_of_step": flux_ms / tot_k,
                 "peak_source": peak_src,
