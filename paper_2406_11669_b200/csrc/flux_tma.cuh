@@ -29,6 +29,9 @@ constexpr int FT_THREADS = 128;
 constexpr int FT_TC = 4;
 constexpr int FT_SLOTS = 3;
 constexpr int FT_NMET = 10;
+#ifndef FT_MINB
+#define FT_MINB 3
+#endif
 
 template <int D>
 struct FtSmem {
@@ -291,7 +294,7 @@ __device__ __forceinline__ void ft_ld4(const double* p, double& a, double& b, do
 // multiple of 4).  For D = 0 the march starts at face -2 so that every 4-cell group of a row
 // is one 32-byte sector.
 template <int D, int RECON>
-__global__ void __launch_bounds__(FT_THREADS, 3)
+__global__ void __launch_bounds__(FT_THREADS, FT_MINB)
 k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
            const __grid_constant__ CUtensorMap tmMet, const __grid_constant__ CUtensorMap tmBf) {
   using Smem = FtSmem<D>;
