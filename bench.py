@@ -197,6 +197,23 @@ ALG_BYTES = {  # algorithmic bytes per interior cell and launch (DESIGN.md "Roof
 }
 
 
+def max_over_ranks(ms, world, device):
+    """Device time of the job = max over the ranks' own times (one block per rank, no data-path
+    collective: "replicas only").  Works on any backend (nccl on the GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(ncells, stages, steps, world, ms):
+    """zone-updates/s per RK substep of all replicas together."""
+    return world * ncells * stages * steps / (ms * 1e-3)
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -250,12 +267,9 @@ def run_b200(args):
     kt = s.kernel_times()
     s.set_option("kernel_timing", 0)
     st = s.stats()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     zone_sub = w.ncells * w.stages * args.steps
-    value = world * zone_sub / (ms * 1e-3)
+    value = whole_job_value(w.ncells, w.stages, args.steps, world, ms)
 
     # ---- end to end through the C ABI with host buffers --------------------------------
     k_e2e = max(1, min(args.steps, 5))
@@ -272,10 +286,7 @@ def run_b200(args):
     barrier()
     wall_e2e = time.perf_counter() - t0
     ms_e2e = max(e0.elapsed_time(e1), 0.0)
-    if world > 1:
-        t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
+    ms_e2e = max_over_ranks(ms_e2e, world, dev)
     h2d = sum(a.numel() * 8 for a in h_prims if a is not None) + \
         (sum(a.numel() * 8 for a in h_vec) if h_vec else 0)
     d2h = sum(a.numel() * 8 for a in out_host)
