@@ -92,13 +92,14 @@ __device__ __forceinline__ double ft_sel(bool c, double a, double b) {
 }
 
 // G8(a): monotonised-central slope from the two one-sided differences.  For same-signed
-// dm, dp the candidates d = (dp+dm)/2 and 2 min(|dp|,|dm|) carry the sign of d already.
+// dm, dp the candidates d = (dp+dm)/2 and 2 min(|dp|,|dm|) carry the sign of d already; if
+// one of them is zero so is the candidate chosen, so "dp dm > 0" reduces to a sign-bit test.
 __device__ __forceinline__ double ft_slope(double dm, double dp) {
   const double d = 0.5 * (dp + dm);
   const double m = fabs(dp) < fabs(dm) ? dp : dm;
   const double m2 = m + m;
   const double r = fabs(d) < fabs(m2) ? d : m2;
-  return dp * dm > 0.0 ? r : 0.0;
+  return ft_opposite(dp, dm) ? 0.0 : r;
 }
 
 template <int RECON>
@@ -145,7 +146,8 @@ struct FtMarch {
       // |a| > 2|b| -> q^+ = q + 2b
       const double a = qp - qa, b = qa - qm;
       const double aa = fabs(a), ab = fabs(b);
-      const bool flat = a * b <= 0.0;
+      // a b <= 0: with a = 0 or b = 0 the two fixes below give q as well, so the sign bits decide
+      const bool flat = ft_opposite(a, b);
       const bool fixm = ab > 2.0 * aa;
       const bool fixp = aa > 2.0 * ab;
       const double qm2 = fma(-2.0, a, qa);

@@ -53,7 +53,7 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
     }
     const double a = qp - q, b = q - qm;
     const double aa = fabs(a), ab = fabs(b);
-    const bool flat = a * b <= 0.0;
+    const bool flat = ft_opposite(a, b);
     const bool fixm = ab > 2.0 * aa;
     const bool fixp = aa > 2.0 * ab;
     const double qm2 = fma(-2.0, a, q);
