@@ -286,13 +286,132 @@ void recon_face(int d, const double c[8][6], const ref_opts& o, double PL[8], do
   }
 }
 
+// ------------------------------------------------------- con2prim, 1-D backup scheme (F4)
+// Palenzuela et al. 1-D scheme: eqs (42)-(45), unknown x = h W, root of
+// eq. (43) f(x) = x - h^ W^ bracketed by 1 + q - s < x < 2 + 2q - s and found with Brent's
+// method (bracketing; no derivative).  Ideal fluid only (eq. 46), so Y_e of eq. (43) is unused.
+// Readings (G23-G25): eq. (45) prints t^2/x where the reduction of eq. (40b) gives
+// t^2/x^2 (z = D x); PAPER.md:315 prints "v^2 = 1 1/W^2" for v^2 = 1 - 1/W^2; 1/W^2 of eq. (44)
+// is kept inside [1/w_max^2, 1] and eps^ is not allowed below 0 while iterating; the lower
+// end of the bracket is raised to 1 when 1 + q - s < 1 (h W >= 1 always).
+struct C2P1D {
+  double q, r, s, t, D, Gamma, iw2min;
+  // eq. (44): 1/W^2 from x
+  double w2inv(double x) const {
+    double v = 1.0 - (r * x * x + t * t * (2.0 * x + s)) / (x * x * sq(x + s));
+    return std::min(std::max(v, iw2min), 1.0);
+  }
+  // eqs (44), (45): W^, eps^ from x
+  void state(double x, double& W, double& eps) const {
+    const double iw2 = w2inv(x);
+    W = 1.0 / std::sqrt(iw2);
+    eps = -1.0 + x / W * (1.0 - W * W) +
+          W * (1.0 + q - s + 0.5 * (t * t / (x * x) + s * iw2));
+    eps = std::max(eps, 0.0);
+  }
+  // eq. (43) with h^ = 1 + eps^ + p^/rho^ = 1 + Gamma eps^ (eq. 46)
+  double f(double x) const {
+    double W, eps;
+    state(x, W, eps);
+    return x - (1.0 + Gamma * eps) * W;
+  }
+};
+
+// Brent's method on [a, b] with f(a) f(b) < 0: inverse quadratic interpolation / secant steps
+// accepted only while they stay well inside the bracket and shrink fast enough, bisection
+// otherwise.  Returns false if the root is not bracketed or maxit is exceeded.
+template <class F>
+bool brent(const F& f, double a, double b, double rtol, int maxit, double& root, int& iters) {
+  double fa = f(a), fb = f(b);
+  iters = 0;
+  if (!(fa * fb < 0.0)) {
+    if (fa == 0.0) { root = a; return true; }
+    if (fb == 0.0) { root = b; return true; }
+    return false;
+  }
+  double c = a, fc = fa, d = b - a, e = d;
+  for (int it = 1; it <= maxit; it++) {
+    iters = it;
+    if ((fb > 0.0) == (fc > 0.0)) { c = a; fc = fa; d = b - a; e = d; }  // keep the root in [b, c]
+    if (std::fabs(fc) < std::fabs(fb)) { a = b; b = c; c = a; fa = fb; fb = fc; fc = fa; }
+    const double tol1 = 2.0 * 2.220446049250313e-16 * std::fabs(b) + 0.5 * rtol * std::fabs(b);
+    const double xm = 0.5 * (c - b);
+    if (std::fabs(xm) <= tol1 || fb == 0.0) { root = b; return true; }
+    if (std::fabs(e) >= tol1 && std::fabs(fa) > std::fabs(fb)) {
+      const double sv = fb / fa;
+      double pp, qq;
+      if (a == c) {  // secant
+        pp = 2.0 * xm * sv;
+        qq = 1.0 - sv;
+      } else {  // inverse quadratic interpolation
+        const double qa = fa / fc, rr = fb / fc;
+        pp = sv * (2.0 * xm * qa * (qa - rr) - (b - a) * (rr - 1.0));
+        qq = (qa - 1.0) * (rr - 1.0) * (sv - 1.0);
+      }
+      if (pp > 0.0) qq = -qq;
+      pp = std::fabs(pp);
+      if (2.0 * pp < std::min(3.0 * xm * qq - std::fabs(tol1 * qq), std::fabs(e * qq))) {
+        e = d; d = pp / qq;
+      } else {
+        d = xm; e = d;
+      }
+    } else {
+      d = xm; e = d;
+    }
+    a = b; fa = fb;
+    b += std::fabs(d) > tol1 ? d : (xm > 0.0 ? tol1 : -tol1);
+    fb = f(b);
+  }
+  return false;
+}
+
+// Steps (i)-(vii) of PAPER.md:299-320.  In: undensitised D, S_j, tau, B^i, metric.
+// Out: rho, v^i, eps.  Returns false on failure (no bracket, no convergence, non-finite).
+bool con2prim_1d(const double Uin[5], const double B[3], const Metric& M, const ref_opts& o,
+                 double& rho, double v[3], double& eps, int* iters_out) {
+  const double D = Uin[0], tau = Uin[4];
+  const double* S = Uin + 1;
+  double gu[3][3];
+  inv3(M.g, det3(M.g), gu);
+  double S2 = 0, B2 = 0, BS = 0;
+  for (int i = 0; i < 3; i++) {
+    for (int j = 0; j < 3; j++) {
+      S2 += gu[i][j] * S[i] * S[j];
+      B2 += M.g[i][j] * B[i] * B[j];
+    }
+    BS += B[i] * S[i];
+  }
+  C2P1D c;  // eq. (42)
+  c.D = D; c.Gamma = o.gamma_ad; c.iw2min = 1.0 / sq(o.w_max);
+  c.q = tau / D; c.r = S2 / (D * D); c.s = B2 / D; c.t = BS / (D * std::sqrt(D));
+  const double lo = std::max(1.0 + c.q - c.s, 1.0), hi = 2.0 + 2.0 * c.q - c.s;
+  int it = 0;
+  double x = 0;
+  const bool ok = hi > lo && brent([&](double xx) { return c.f(xx); }, lo, hi, 1e-14, 100, x, it);
+  if (iters_out) *iters_out = it;
+  if (!ok || !std::isfinite(x)) return false;
+  double W;
+  c.state(x, W, eps);          // (iii), (v)
+  rho = D / W;                 // (iv)
+  const double z = D * x;      // (vii): z = rho W x = rho h W^2
+  for (int i = 0; i < 3; i++) {
+    double Su = 0;
+    for (int j = 0; j < 3; j++) Su += gu[i][j] * S[j];
+    v[i] = Su / (z + B2) + BS * B[i] / (z * (z + B2));  // eq. (41c)
+  }
+  return std::isfinite(rho) && std::isfinite(eps) && std::isfinite(v[0]) &&
+         std::isfinite(v[1]) && std::isfinite(v[2]);
+}
+
 // ------------------------------------------------------------------------- con2prim
 // R14: Noble et al. 2-D Newton-Raphson on (z, v^2), eqs (36)-(41) PAPER.md:260-295, with
 // the atmosphere of PAPER.md:326 and the failure policy G17-G20.
 // In: undensitised D,S_j,tau; B^i; metric.  Out: P5 = rho,v^i,p; U5 = D,S_j,tau (rewritten
 // when a floor or cap was applied).  Returns status bits.
+// `backup`: on a failure of the 2-D scheme try the 1-D scheme above before giving up
+// (PAPER.md:684); status bit 16 marks a state recovered that way.
 int con2prim(const double Uin[5], const double B[3], const Metric& M, const ref_opts& o,
-             bool masked, double P5[5], double U5[5], int* iters_out) {
+             bool masked, double P5[5], double U5[5], int* iters_out, bool backup = false) {
   const double Gamma = o.gamma_ad;
   const double p_atm = std::max(o.poly_k * std::pow(o.rho_atm, o.poly_gamma), o.p_floor);
   const double v2max = 1.0 - 1.0 / sq(o.w_max);
@@ -350,24 +469,33 @@ int con2prim(const double Uin[5], const double B[3], const Metric& M, const ref_
     if (!std::isfinite(err)) break;
     if (err < o.c2p_tol) { converged = true; break; }
   }
-  if (!converged || !std::isfinite(z) || !std::isfinite(v2)) return atmosphere(2);
-
-  // eqs (41a)-(41d); G19: the 1/gamma of (41d) is 1/Gamma.
-  const double W = 1.0 / std::sqrt(1.0 - v2);
-  double rho = D / W;
-  double v[3];
-  for (int i = 0; i < 3; i++) {
-    double Su = 0;
-    for (int j = 0; j < 3; j++) Su += gu[i][j] * S[j];
-    v[i] = Su / (z + B2) + BS * B[i] / (z * (z + B2));
+  bool have = converged && std::isfinite(z) && std::isfinite(v2);
+  double rho = 0, v[3] = {0, 0, 0}, eps = 0, p = 0;
+  if (have) {
+    // eqs (41a)-(41d); G19: the 1/gamma of (41d) is 1/Gamma.
+    const double W = 1.0 / std::sqrt(1.0 - v2);
+    rho = D / W;
+    for (int i = 0; i < 3; i++) {
+      double Su = 0;
+      for (int j = 0; j < 3; j++) Su += gu[i][j] * S[j];
+      v[i] = Su / (z + B2) + BS * B[i] / (z * (z + B2));
+    }
+    eps = (z / (rho * W * W) - 1.0) / Gamma;
+    p = (Gamma - 1.0) * rho * eps;
+    have = std::isfinite(rho) && std::isfinite(p) && std::isfinite(v[0]) &&
+           std::isfinite(v[1]) && std::isfinite(v[2]) && !(rho < o.rho_atm);
   }
-  double eps = (z / (rho * W * W) - 1.0) / Gamma;
-  double p = (Gamma - 1.0) * rho * eps;
-  if (!std::isfinite(rho) || !std::isfinite(p) || !std::isfinite(v[0]) ||
-      !std::isfinite(v[1]) || !std::isfinite(v[2]) || rho < o.rho_atm)
-    return atmosphere(2);
-
   int bits = 0;
+  if (!have) {
+    int it1 = 0;
+    if (backup && con2prim_1d(Uin, B, M, o, rho, v, eps, &it1) && !(rho < o.rho_atm)) {
+      p = (Gamma - 1.0) * rho * eps;
+      bits |= 16;
+    } else {
+      return atmosphere(2);
+    }
+  }
+
   bool rewrite = false;
   if (eps < 0.0 || p < o.p_floor) {  // G20 (ii): pressure fix, keep rho and v
     p = o.p_floor;
@@ -484,6 +612,8 @@ struct ref_grmhd {
   bool have_metric = false, have_prims = false, have_mask = false;
   double t = 0, dt = 0, fixed_dt = 0, maxspeed[3] = {0, 0, 0};
   long long steps = 0, c2p_fail = 0, p_fix = 0, atmo = 0, w_cap = 0, c2p_maxiter = 0;
+  long long c2p_backup_used = 0;
+  int c2p_backup = 0;  // option: 1-D scheme on a failure of the 2-D one
   bool bad_dt = false;
 
   size_t idx(int i, int j, int k) const {
@@ -618,8 +748,8 @@ struct ref_grmhd {
 
   // ------------------------------------------------- con2prim over the interior (R14)
   void recover_primitives() {
-    long long nf = 0, np = 0, na = 0, nw = 0, mi = 0;
-#pragma omp parallel for num_threads(g_threads) reduction(+ : nf, np, na, nw) reduction(max : mi)
+    long long nf = 0, np = 0, na = 0, nw = 0, nb = 0, mi = 0;
+#pragma omp parallel for num_threads(g_threads) reduction(+ : nf, np, na, nw, nb) reduction(max : mi)
     for (int k = 0; k < nz; k++)
       for (int j = 0; j < ny; j++)
         for (int i = 0; i < nx; i++) {
@@ -630,17 +760,18 @@ struct ref_grmhd {
           for (int r = 0; r < 5; r++) Uin[r] = U[r][c] / sg;  // undensitise, eq. (17)
           for (int d = 0; d < 3; d++) B[d] = Bc[d][c];
           int it = 0;
-          const int bits = con2prim(Uin, B, M, o, have_mask && mask[c], P5, U5, &it);
+          const int bits = con2prim(Uin, B, M, o, have_mask && mask[c], P5, U5, &it,
+                                    c2p_backup != 0);
           for (int r = 0; r < 5; r++) P[r][c] = P5[r];
-          if (bits) {
+          if (bits & (1 | 2 | 4 | 8)) {
             if (bits & (1 | 2 | 8)) U[0][c] = sg * U5[0];
             for (int r = 1; r < 5; r++) U[r][c] = sg * U5[r];
           }
           nf += (bits & 2) != 0; np += (bits & 4) != 0; na += (bits & 1) != 0;
-          nw += (bits & 8) != 0;
+          nw += (bits & 8) != 0; nb += (bits & 16) != 0;
           if (it > mi) mi = it;
         }
-    c2p_fail += nf; p_fix += np; atmo += na; w_cap += nw;
+    c2p_fail += nf; p_fix += np; atmo += na; w_cap += nw; c2p_backup_used += nb;
     c2p_maxiter = std::max(c2p_maxiter, mi);
   }
 
@@ -982,7 +1113,7 @@ int ref_set_prims(ref_grmhd* h, const double* const field[8]) {
   }
   h->have_prims = true;
   h->t = 0; h->steps = 0; h->dt = 0;
-  h->c2p_fail = h->p_fix = h->atmo = h->w_cap = h->c2p_maxiter = 0;
+  h->c2p_fail = h->p_fix = h->atmo = h->w_cap = h->c2p_maxiter = h->c2p_backup_used = 0;
   h->bad_dt = false;
   init_state_from_prims(h);
   return 0;
@@ -1075,6 +1206,7 @@ int ref_get_bface(ref_grmhd* h, double* const field[3]) {
 int ref_set_option(ref_grmhd* h, const char* key, double value) {
   if (!h || !key) return -1;
   if (std::strcmp(key, "fixed_dt") == 0) { h->fixed_dt = value; return 0; }
+  if (std::strcmp(key, "c2p_backup") == 0) { h->c2p_backup = value != 0.0; return 0; }
   return -1;
 }
 
@@ -1084,6 +1216,7 @@ int ref_get_stats(ref_grmhd* h, ref_stats* out) {
   for (int d = 0; d < 3; d++) out->maxspeed[d] = h->maxspeed[d];
   out->steps = h->steps; out->c2p_fail = h->c2p_fail; out->p_fix = h->p_fix;
   out->atmo = h->atmo; out->w_cap = h->w_cap; out->c2p_maxiter = h->c2p_maxiter;
+  out->c2p_backup = h->c2p_backup_used;
   return h->bad_dt ? -5 : 0;
 }
 
@@ -1116,6 +1249,42 @@ int ref_con2prim_pt(const double cons[8], const double metric[10], const ref_opt
                     int masked, double prim_out[5], double cons_out[5], int* iters) {
   return con2prim(cons, cons + 5, unpack_metric(metric), *o, masked != 0, prim_out, cons_out,
                   iters);
+}
+
+int ref_con2prim_backup_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                           double prim_out[5], double cons_out[5], int* iters) {
+  return con2prim(cons, cons + 5, unpack_metric(metric), *o, false, prim_out, cons_out, iters,
+                  true);
+}
+
+int ref_con2prim1d_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                      double prim_out[5], int* iters) {
+  double rho, v[3], eps;
+  const bool ok = con2prim_1d(cons, cons + 5, unpack_metric(metric), *o, rho, v, eps, iters);
+  prim_out[0] = rho; prim_out[1] = v[0]; prim_out[2] = v[1]; prim_out[3] = v[2];
+  prim_out[4] = (o->gamma_ad - 1.0) * rho * eps;
+  return ok ? 0 : 2;
+}
+
+void ref_c2p1d_relations_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                            double x, double out[3]) {
+  // eq. (44) -> W^, eq. (45) -> eps^, eq. (43) -> f at a given x: pins of the restatement
+  const Metric M = unpack_metric(metric);
+  double gu[3][3];
+  inv3(M.g, det3(M.g), gu);
+  const double* S = cons + 1;
+  const double* B = cons + 5;
+  double S2 = 0, B2 = 0, BS = 0;
+  for (int i = 0; i < 3; i++) {
+    for (int j = 0; j < 3; j++) { S2 += gu[i][j] * S[i] * S[j]; B2 += M.g[i][j] * B[i] * B[j]; }
+    BS += B[i] * S[i];
+  }
+  const double D = cons[0];
+  C2P1D c;
+  c.D = D; c.Gamma = o->gamma_ad; c.iw2min = 1.0 / sq(o->w_max);
+  c.q = cons[4] / D; c.r = S2 / (D * D); c.s = B2 / D; c.t = BS / (D * std::sqrt(D));
+  c.state(x, out[0], out[1]);
+  out[2] = c.f(x);
 }
 
 void ref_flux_pt(int d, const double prim[8], const double metric[10], double gamma_ad,

@@ -28,6 +28,7 @@ typedef struct {
 typedef struct {
   double t, dt, maxspeed[3];
   long long steps, c2p_fail, p_fix, atmo, w_cap, c2p_maxiter;
+  long long c2p_backup; /* states recovered by the 1-D backup scheme (option "c2p_backup") */
 } ref_stats;
 
 int ref_create(int nx, int ny, int nz, int ghosts, const double dx[3], const ref_opts* o,
@@ -65,6 +66,16 @@ void ref_prim2con_pt(const double prim[8], const double metric[10], double gamma
  * (possibly rewritten) undensitised D,S_j,tau */
 int ref_con2prim_pt(const double cons[8], const double metric[10], const ref_opts* o,
                     int masked, double prim_out[5], double cons_out[5], int* iters);
+/* as ref_con2prim_pt with the 1-D backup enabled (status bit 16 = recovered by the backup) */
+int ref_con2prim_backup_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                           double prim_out[5], double cons_out[5], int* iters);
+/* the 1-D scheme alone, eqs (42)-(45) PAPER.md:297-320: prim_out = rho, v^i, p without floors;
+ * returns 0 or 2 (no bracket / no convergence); iters = Brent iterations */
+int ref_con2prim1d_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                      double prim_out[5], int* iters);
+/* out = W^ of eq. (44), eps^ of eq. (45), f of eq. (43) at a given x */
+void ref_c2p1d_relations_pt(const double cons[8], const double metric[10], const ref_opts* o,
+                            double x, double out[3]);
 void ref_flux_pt(int d, const double prim[8], const double metric[10], double gamma_ad,
                  double F[8]); /* eq. (18), including its 1/alpha */
 void ref_speeds_pt(int d, const double prim[8], const double metric[10], double gamma_ad,

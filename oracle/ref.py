@@ -41,7 +41,8 @@ class RefOpts(C.Structure):
 class RefStats(C.Structure):
     _fields_ = [("t", C.c_double), ("dt", C.c_double), ("maxspeed", C.c_double * 3),
                 ("steps", C.c_longlong), ("c2p_fail", C.c_longlong), ("p_fix", C.c_longlong),
-                ("atmo", C.c_longlong), ("w_cap", C.c_longlong), ("c2p_maxiter", C.c_longlong)]
+                ("atmo", C.c_longlong), ("w_cap", C.c_longlong), ("c2p_maxiter", C.c_longlong),
+                ("c2p_backup", C.c_longlong)]
 
 
 def make_opts(gamma_ad=5.0 / 3.0, poly_k=1.0, poly_gamma=None, rho_atm=1e-10, p_floor=1e-12,
@@ -214,6 +215,33 @@ def con2prim_pt(cons, metric, opts: RefOpts, masked=0):
     bits = lib().ref_con2prim_pt(_dp(_v(cons, 8)), _dp(_v(metric, 10)), C.byref(opts),
                                  int(masked), _dp(p), _dp(u), C.byref(it))
     return p, u, bits, it.value
+
+
+def con2prim_backup_pt(cons, metric, opts: RefOpts):
+    """2-D scheme with the 1-D backup enabled; status bit 16 = recovered by the backup."""
+    p = np.zeros(5)
+    u = np.zeros(5)
+    it = C.c_int(0)
+    bits = lib().ref_con2prim_backup_pt(_dp(_v(cons, 8)), _dp(_v(metric, 10)), C.byref(opts),
+                                        _dp(p), _dp(u), C.byref(it))
+    return p, u, bits, it.value
+
+
+def con2prim1d_pt(cons, metric, opts: RefOpts):
+    """The 1-D scheme alone (eqs 42-45): (rho, v^i, p), status 0 / 2, Brent iterations."""
+    p = np.zeros(5)
+    it = C.c_int(0)
+    st = lib().ref_con2prim1d_pt(_dp(_v(cons, 8)), _dp(_v(metric, 10)), C.byref(opts), _dp(p),
+                                 C.byref(it))
+    return p, st, it.value
+
+
+def c2p1d_relations_pt(cons, metric, opts: RefOpts, x):
+    """(W^ of eq. 44, eps^ of eq. 45, f of eq. 43) at a given x = h W."""
+    out = np.zeros(3)
+    lib().ref_c2p1d_relations_pt(_dp(_v(cons, 8)), _dp(_v(metric, 10)), C.byref(opts),
+                                 C.c_double(x), _dp(out))
+    return out
 
 
 def flux_pt(d, prim, metric, gamma_ad):
