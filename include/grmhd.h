@@ -83,6 +83,7 @@ typedef struct {
   long long atmo;       /* cell-substeps reset because D <= rho_atm or masked              */
   long long w_cap;      /* cell-substeps whose velocity was rescaled to w_max              */
   long long c2p_maxiter;/* largest Newton iteration count seen                             */
+  long long c2p_backup; /* cell-substeps recovered by the 1-D backup scheme ("c2p_backup")  */
 } grmhd_stats;
 
 /* Bytes of DEVICE workspace the handle needs for this block (0 on invalid arguments). */
@@ -136,6 +137,11 @@ int grmhd_get_cons(grmhd* h, double* const field[8]);
 int grmhd_get_vecpot(grmhd* h, double* const field[3]);
 
 /* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off);
+ * "c2p_backup" (1: when the 2-D Newton con2prim fails, try the 1-D scheme of PAPER.md:297-320,
+ * eqs (42)-(45), before resetting the cell to atmosphere -- the paper's policy, PAPER.md:684;
+ * 0 = off, the default: failure -> atmosphere, G20);
+ * "flux_kernel" (1 default: TMA-fed kernels; 0: the all-register marching kernel everywhere),
+ * "flux_x_rows" (1 default: lanes-along-x kernel for the x fluxes; 0: as y and z);
  * "kernel_timing" (1: bracket every kernel group of the step with CUDA events on the
  * handle's stream and accumulate device times, see grmhd_get_kernel_times; 0 = off;
  * setting it clears the accumulators).  Unknown key -> EINVAL. */
@@ -171,6 +177,12 @@ int grmhd_prim2con_batch(const double* const prim[8], const double* const metric
 int grmhd_con2prim_batch(const double* const cons[8], const double* const metric[10],
                          double* const prim[5], int* status, int* iters, long long n,
                          const grmhd_opts* opts, void* stream);
+/* The 1-D scheme alone (eqs 42-45; Brent's method on x = hW): prim out =
+ * rho, v^i, p = (Gamma-1) rho eps without floors; status 0 = converged, 2 = no bracket / no
+ * convergence; iters = Brent iterations. */
+int grmhd_con2prim1d_batch(const double* const cons[8], const double* const metric[10],
+                           double* const prim[5], int* status, int* iters, long long n,
+                           const grmhd_opts* opts, void* stream);
 /* Dependent-free DFMA loop used to MEASURE the FP64 pipe peak: each of `threads` threads
  * performs `iters` * 16 DFMAs; out receives one double per thread.  */
 int grmhd_dfma_peak(double* out, long long threads, int iters, void* stream);

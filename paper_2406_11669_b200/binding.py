@@ -23,7 +23,7 @@ EXPORTS = ["grmhd_workspace_bytes", "grmhd_create", "grmhd_destroy", "grmhd_set_
            "grmhd_set_prims", "grmhd_set_vecpot", "grmhd_set_mask", "grmhd_step",
            "grmhd_step_until", "grmhd_get_prims", "grmhd_get_cons", "grmhd_get_vecpot",
            "grmhd_set_option", "grmhd_get_stats", "grmhd_get_kernel_times", "grmhd_launch_count", "grmhd_last_error",
-           "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_dfma_peak"]
+           "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_con2prim1d_batch", "grmhd_dfma_peak"]
 
 
 class GrmhdOpts(C.Structure):
@@ -37,7 +37,8 @@ class GrmhdOpts(C.Structure):
 class GrmhdStats(C.Structure):
     _fields_ = [("t", C.c_double), ("dt", C.c_double), ("maxspeed", C.c_double * 3),
                 ("steps", C.c_longlong), ("c2p_fail", C.c_longlong), ("p_fix", C.c_longlong),
-                ("atmo", C.c_longlong), ("w_cap", C.c_longlong), ("c2p_maxiter", C.c_longlong)]
+                ("atmo", C.c_longlong), ("w_cap", C.c_longlong), ("c2p_maxiter", C.c_longlong),
+                ("c2p_backup", C.c_longlong)]
 
 
 class GrmhdError(RuntimeError):
@@ -289,6 +290,23 @@ def con2prim_batch(cons, metric, opts: GrmhdOpts):
                                     C.c_void_p(torch.cuda.current_stream().cuda_stream))
     if rc != OK:
         raise GrmhdError("grmhd_con2prim_batch", rc)
+    return prim, status, iters
+
+
+def con2prim1d_batch(cons, metric, opts: GrmhdOpts):
+    """The 1-D backup scheme alone: cons (8,n), metric (10,n) -> prim (5,n), status, iters."""
+    _require_cuda()
+    n = cons.shape[1]
+    prim = torch.empty((5, n), dtype=torch.float64, device=cons.device)
+    status = torch.empty(n, dtype=torch.int32, device=cons.device)
+    iters = torch.empty(n, dtype=torch.int32, device=cons.device)
+    keep = []
+    rc = lib().grmhd_con2prim1d_batch(_ptrs(list(cons), 8, keep), _ptrs(list(metric), 10, keep),
+                                      _ptrs(list(prim), 5, keep), C.c_void_p(status.data_ptr()),
+                                      C.c_void_p(iters.data_ptr()), n, C.byref(opts),
+                                      C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if rc != OK:
+        raise GrmhdError("grmhd_con2prim1d_batch", rc)
     return prim, status, iters
 
 

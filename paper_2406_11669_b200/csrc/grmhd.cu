@@ -140,6 +140,7 @@ Eos make_eos(const grmhd_opts& o) {
   E.recon = o.recon;
   E.flatten = o.ppm_flatten;
   E.riemann = o.riemann;
+  E.c2p_backup = 0;
   return E;
 }
 
@@ -270,8 +271,12 @@ int after_stage(grmhd* h, bool want_speed) {
     if (rc) return rc;
   });
   KT(KG_C2P, {
-    k_post<false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
-        h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+    if (h->E.c2p_backup)
+      k_post<false, true><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
+          h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+    else
+      k_post<false, false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
+          h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
     CKL("k_post");
   });
   KT(KG_SRC, {
@@ -490,7 +495,7 @@ int init_state(grmhd* h) {
   if (rc) return rc;
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 0);
   CKL("k_reset_state");
-  k_post<true><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
+  k_post<true, false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
       h->base, nullptr, g, h->E, h->dst, 1);
   CKL("k_post");
   k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
@@ -718,6 +723,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
     h->flux_impl = (int)value;
     return GRMHD_OK;
   }
+  if (std::strcmp(key, "c2p_backup") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: c2p_backup is 0 or 1");
+    h->E.c2p_backup = (int)value;
+    return GRMHD_OK;
+  }
   if (std::strcmp(key, "flux_x_rows") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_x_rows is 0 or 1");
     h->xrow = (int)value;
@@ -752,6 +762,7 @@ int grmhd_get_stats(grmhd* h, grmhd_stats* out) {
   out->steps = h->steps;
   out->c2p_fail = st.c2p_fail; out->p_fix = st.p_fix; out->atmo = st.atmo;
   out->w_cap = st.w_cap; out->c2p_maxiter = st.c2p_maxiter;
+  out->c2p_backup = st.c2p_backup;
   if (st.bad_dt) return fail(h, GRMHD_ENUMERIC, "dt not finite/positive");
   return GRMHD_OK;
 }
@@ -795,6 +806,21 @@ int grmhd_con2prim_batch(const double* const cons[8], const double* const metric
   for (int r = 0; r < 5; r++) { if (!prim[r]) return GRMHD_EINVAL; bp.cons[r] = prim[r]; }
   if (n == 0) return GRMHD_OK;
   k_con2prim_batch<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
+      bp, status, iters, n, make_eos(*opts));
+  return cudaGetLastError() == cudaSuccess ? GRMHD_OK : GRMHD_ECUDA;
+}
+
+int grmhd_con2prim1d_batch(const double* const cons[8], const double* const metric[10],
+                           double* const prim[5], int* status, int* iters, long long n,
+                           const grmhd_opts* opts, void* stream) {
+  if (!cons || !metric || !prim || !status || !iters || n < 0 || !valid_opts(opts))
+    return GRMHD_EINVAL;
+  BatchPtrs bp{};
+  for (int r = 0; r < 8; r++) { if (!cons[r]) return GRMHD_EINVAL; bp.prim[r] = cons[r]; }
+  for (int r = 0; r < 10; r++) { if (!metric[r]) return GRMHD_EINVAL; bp.met[r] = metric[r]; }
+  for (int r = 0; r < 5; r++) { if (!prim[r]) return GRMHD_EINVAL; bp.cons[r] = prim[r]; }
+  if (n == 0) return GRMHD_OK;
+  k_con2prim1d_batch<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
       bp, status, iters, n, make_eos(*opts));
   return cudaGetLastError() == cudaSuccess ? GRMHD_OK : GRMHD_ECUDA;
 }

@@ -409,7 +409,7 @@ constexpr int KP_THREADS = 32 * KP_BY * KP_BZ;
 #ifndef KP_MINB
 #define KP_MINB 5
 #endif
-template <bool INIT>
+template <bool INIT, bool BACKUP>
 __global__ void __launch_bounds__(KP_THREADS, KP_MINB)
 k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
        DevState* __restrict__ st, int want_speed) {
@@ -468,7 +468,8 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
 #pragma unroll
       for (int r = 0; r < 5; r++) U[r] = fld(base, g, F_Y + r)[c] * isg;  // undensitise, eq. (17)
       int rewrite;
-      bits = con2prim(U, Bx, By, Bz, M, E, mask != nullptr && mask[c] != 0, P5, iters, rewrite);
+      bits = con2prim<BACKUP>(U, Bx, By, Bz, M, E, mask != nullptr && mask[c] != 0, P5, iters,
+                              rewrite);
 #pragma unroll
       for (int r = 0; r < 5; r++) fld(base, g, F_P + r)[c] = P5[r];
       if (rewrite & 1) fld(base, g, F_Y + 0)[c] = sg * U[0];
@@ -488,11 +489,13 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
       const int np = __popc(__ballot_sync(0xffffffffu, (bits & 4) != 0));
       const int na = __popc(__ballot_sync(0xffffffffu, (bits & 1) != 0));
       const int nw = __popc(__ballot_sync(0xffffffffu, (bits & 8) != 0));
+      const int nb = __popc(__ballot_sync(0xffffffffu, (bits & 16) != 0));
       if (threadIdx.x == 0) {
         if (nf) atomicAdd((unsigned long long*)&st->c2p_fail, (unsigned long long)nf);
         if (np) atomicAdd((unsigned long long*)&st->p_fix, (unsigned long long)np);
         if (na) atomicAdd((unsigned long long*)&st->atmo, (unsigned long long)na);
         if (nw) atomicAdd((unsigned long long*)&st->w_cap, (unsigned long long)nw);
+        if (nb) atomicAdd((unsigned long long*)&st->c2p_backup, (unsigned long long)nb);
       }
     }
     int mi = iters;

@@ -14,7 +14,7 @@ __global__ void k_reset_state(DevState* st, int full) {
   for (int d = 0; d < 3; d++) st->ms_acc[d] = 0ull;
   if (full) {
     st->t = 0.0; st->dt = 0.0;
-    st->c2p_fail = st->p_fix = st->atmo = st->w_cap = st->c2p_maxiter = 0;
+    st->c2p_fail = st->p_fix = st->atmo = st->w_cap = st->c2p_maxiter = st->c2p_backup = 0;
     st->bad_dt = 0;
   }
 }
@@ -59,6 +59,22 @@ k_con2prim_batch(BatchPtrs b, int* __restrict__ status, int* __restrict__ iters,
 #pragma unroll
   for (int r = 0; r < 5; r++) b.cons[r][q] = P5[r];
   status[q] = bits;
+  iters[q] = it;
+}
+
+__global__ void __launch_bounds__(128)
+k_con2prim1d_batch(BatchPtrs b, int* __restrict__ status, int* __restrict__ iters, long long n,
+                   Eos E) {
+  const long long q = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (q >= n) return;
+  const double U[5] = {b.prim[0][q], b.prim[1][q], b.prim[2][q], b.prim[3][q], b.prim[4][q]};
+  double rho = 0, vx = 0, vy = 0, vz = 0, eps = 0;
+  int it = 0;
+  const bool ok = con2prim_1d(U, b.prim[5][q], b.prim[6][q], b.prim[7][q], batch_met(b, q), E,
+                              rho, vx, vy, vz, eps, it);
+  b.cons[0][q] = rho; b.cons[1][q] = vx; b.cons[2][q] = vy; b.cons[3][q] = vz;
+  b.cons[4][q] = (E.Gamma - 1.0) * rho * eps;
+  status[q] = ok ? 0 : 2;
   iters[q] = it;
 }
 

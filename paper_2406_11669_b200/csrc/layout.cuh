@@ -58,6 +58,7 @@ struct DevState {
   unsigned long long ms_acc[3];      // bit patterns of max |lambda| per direction (A8)
   double ms_used[3];                 // speeds the last dt was computed from
   long long c2p_fail, p_fix, atmo, w_cap, c2p_maxiter;
+  long long c2p_backup;              // states recovered by the 1-D backup scheme
   int bad_dt;
   int pad;
 };

@@ -82,11 +82,107 @@ __device__ __forceinline__ void recon_pair(int recon, const double c[6], double 
   }
 }
 
+// --------------------------------------------------------- con2prim, 1-D backup scheme
+// Row F4: the scheme of PAPER.md:297-320 (eqs 42-45) the paper falls back to when the 2-D
+// Newton iteration fails.  One unknown x = h W, bracketed by
+// max(1 + q - s, 1) < x < 2 + 2q - s, root of eq. (43) by Brent's method.  Readings G23-G25 of
+// DESIGN.md (t^2/x^2 in eq. (45); 1/W^2 kept in [1/w_max^2, 1]; eps^ >= 0 while iterating).
+// Rare path: plain IEEE division and square root, not inlined.
+struct C2p1d {
+  double q, r, s, t, Gamma, iw2min;
+  __device__ void state(double x, double& W, double& eps) const {
+    double iw2 = 1.0 - (r * x * x + t * t * (2.0 * x + s)) / (x * x * (x + s) * (x + s));  // (44)
+    iw2 = fmin(fmax(iw2, iw2min), 1.0);
+    W = 1.0 / sqrt(iw2);
+    eps = -1.0 + x / W * (1.0 - W * W) +
+          W * (1.0 + q - s + 0.5 * (t * t / (x * x) + s * iw2));  // (45)
+    eps = fmax(eps, 0.0);
+  }
+  __device__ double f(double x) const {  // (43), h^ = 1 + Gamma eps^ for the ideal fluid
+    double W, eps;
+    state(x, W, eps);
+    return x - (1.0 + Gamma * eps) * W;
+  }
+};
+
+// U = undensitised (D, S_j, tau).  Returns true and rho, v^i, eps on success.
+__device__ __noinline__ bool con2prim_1d(const double* U, double Bx, double By, double Bz,
+                                         const Met& M, const Eos& E, double& rho, double& vx,
+                                         double& vy, double& vz, double& eps, int& iters) {
+  const double D = U[0], Sx = U[1], Sy = U[2], Sz = U[3], tau = U[4];
+  const double idet = 1.0 / det_gamma(M);
+  const Sym3 gu = inv_gamma(M, idet);
+  const double Sux = gu.xx * Sx + gu.xy * Sy + gu.xz * Sz;
+  const double Suy = gu.xy * Sx + gu.yy * Sy + gu.yz * Sz;
+  const double Suz = gu.xz * Sx + gu.yz * Sy + gu.zz * Sz;
+  const double S2 = Sux * Sx + Suy * Sy + Suz * Sz;
+  double Blx, Bly, Blz;
+  lower(M, Bx, By, Bz, Blx, Bly, Blz);
+  const double B2 = Blx * Bx + Bly * By + Blz * Bz;
+  const double BS = Bx * Sx + By * Sy + Bz * Sz;
+  C2p1d c;  // eq. (42)
+  c.Gamma = E.Gamma; c.iw2min = 1.0 - E.v2max;
+  c.q = tau / D; c.r = S2 / (D * D); c.s = B2 / D; c.t = BS / (D * sqrt(D));
+  double a = fmax(1.0 + c.q - c.s, 1.0), b = 2.0 + 2.0 * c.q - c.s;
+  iters = 0;
+  if (!(b > a)) return false;
+  // Brent: bracket [b, cc] with |f(b)| <= |f(cc)|, a = previous iterate
+  double fa = c.f(a), fb = c.f(b);
+  bool found = false;
+  double x = 0.0;
+  if (fa == 0.0) { x = a; found = true; }
+  else if (fb == 0.0) { x = b; found = true; }
+  else if (!(fa * fb < 0.0)) return false;
+  double cc = a, fc = fa, d = b - a, e = d;
+  for (int it = 1; it <= 100 && !found; it++) {
+    iters = it;
+    if ((fb > 0.0) == (fc > 0.0)) { cc = a; fc = fa; d = b - a; e = d; }
+    if (fabs(fc) < fabs(fb)) { a = b; b = cc; cc = a; fa = fb; fb = fc; fc = fa; }
+    const double tol1 = 2.0 * 2.220446049250313e-16 * fabs(b) + 0.5 * 1e-14 * fabs(b);
+    const double xm = 0.5 * (cc - b);
+    if (fabs(xm) <= tol1 || fb == 0.0) { x = b; found = true; break; }
+    if (fabs(e) >= tol1 && fabs(fa) > fabs(fb)) {
+      const double sv = fb / fa;
+      double pp, qq;
+      if (a == cc) {
+        pp = 2.0 * xm * sv;
+        qq = 1.0 - sv;
+      } else {
+        const double qa = fa / fc, rr = fb / fc;
+        pp = sv * (2.0 * xm * qa * (qa - rr) - (b - a) * (rr - 1.0));
+        qq = (qa - 1.0) * (rr - 1.0) * (sv - 1.0);
+      }
+      if (pp > 0.0) qq = -qq;
+      pp = fabs(pp);
+      if (2.0 * pp < fmin(3.0 * xm * qq - fabs(tol1 * qq), fabs(e * qq))) { e = d; d = pp / qq; }
+      else { d = xm; e = d; }
+    } else {
+      d = xm; e = d;
+    }
+    a = b; fa = fb;
+    b += fabs(d) > tol1 ? d : (xm > 0.0 ? tol1 : -tol1);
+    fb = c.f(b);
+  }
+  if (!found || !isfinite(x)) return false;
+  double W;
+  c.state(x, W, eps);
+  rho = D / W;
+  const double z = D * x;  // (vii): z = rho W x
+  const double izB = 1.0 / (z + B2), BSz = BS / z;
+  vx = (Sux + BSz * Bx) * izB;  // eq. (41c)
+  vy = (Suy + BSz * By) * izB;
+  vz = (Suz + BSz * Bz) * izB;
+  return isfinite(rho) && isfinite(eps) && isfinite(vx) && isfinite(vy) && isfinite(vz);
+}
+
 // ---------------------------------------------------------------------------- con2prim
 // R14: Noble 2-D Newton-Raphson on (z, v^2), eqs (36)-(41) PAPER.md:260-295; atmosphere
 // PAPER.md:326; failure policy G17-G20.  U = undensitised (D,S_j,tau) in/out, B^i, metric.
 // Returns status bits: 1 atmosphere, 2 failed solve, 4 pressure fix, 8 W cap.
 // `rewrite` mask tells which of U changed: bit0 -> D, bit1 -> S_j and tau.
+// BACKUP (compile time, so that the default kernel carries no call frame): on a failure of
+// the Newton iteration try con2prim_1d before giving up; status bit 16 = recovered that way.
+template <bool BACKUP = false>
 __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, double Bz,
                                         const Met& M, const Eos& E, bool masked, double P5[5],
                                         int& iters, int& rewrite) {
@@ -141,9 +237,9 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
       if (!isfinite(err)) break;
       if (err < E.c2p_tol) { conv = true; break; }
     }
-    if (!conv || !isfinite(z) || !isfinite(v2)) {
-      atmo = true; bits = 2;
-    } else {
+    bool have = conv && isfinite(z) && isfinite(v2);
+    double eps = 0.0;
+    if (have) {
       // eqs (41a)-(41d); G19: the 1/gamma of (41d) is 1/Gamma
       const double iW2 = 1.0 - v2;
       const double iW = iW2 * ft_rsqrt(iW2);
@@ -154,24 +250,33 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
       vy = (Suy + BSz * By) * izB;
       vz = (Suz + BSz * Bz) * izB;
       // z (1 - v^2)/rho = z/(D W)
-      const double eps = (z * iW * ft_rcp(D) - 1.0) * (1.0 - E.gm1oG);
+      eps = (z * iW * ft_rcp(D) - 1.0) * (1.0 - E.gm1oG);
       p = (E.Gamma - 1.0) * rho * eps;
-      if (!isfinite(rho) || !isfinite(p) || !isfinite(vx) || !isfinite(vy) || !isfinite(vz) ||
-          rho < E.rho_atm) {
-        atmo = true; bits = 2;
-      } else {
-        if (eps < 0.0 || p < E.p_floor) {  // G20 (ii): pressure fix, keep rho and v
-          p = E.p_floor;
-          bits |= 4;
-        }
-        double lx, ly, lz;
-        lower(M, vx, vy, vz, lx, ly, lz);
-        const double vv = lx * vx + ly * vy + lz * vz;
-        if (vv > E.v2max) {  // R14 (8): Lorentz-factor cap
-          const double f = sqrt(E.v2max / vv);
-          vx *= f; vy *= f; vz *= f;
-          bits |= 8;
-        }
+      have = isfinite(rho) && isfinite(p) && isfinite(vx) && isfinite(vy) && isfinite(vz) &&
+             !(rho < E.rho_atm);
+    }
+    if (BACKUP && !have) {  // the 1-D scheme as backup (row F4)
+      int it1;
+      if (con2prim_1d(U, Bx, By, Bz, M, E, rho, vx, vy, vz, eps, it1) && !(rho < E.rho_atm)) {
+        p = (E.Gamma - 1.0) * rho * eps;
+        bits |= 16;
+        have = true;
+      }
+    }
+    if (!have) {
+      atmo = true; bits = 2;
+    } else {
+      if (eps < 0.0 || p < E.p_floor) {  // G20 (ii): pressure fix, keep rho and v
+        p = E.p_floor;
+        bits |= 4;
+      }
+      double lx, ly, lz;
+      lower(M, vx, vy, vz, lx, ly, lz);
+      const double vv = lx * vx + ly * vy + lz * vz;
+      if (vv > E.v2max) {  // R14 (8): Lorentz-factor cap
+        const double f = sqrt(E.v2max / vv);
+        vx *= f; vy *= f; vz *= f;
+        bits |= 8;
       }
     }
   }
@@ -179,7 +284,7 @@ __device__ __forceinline__ int con2prim(double U[5], double Bx, double By, doubl
     rho = E.rho_atm; vx = vy = vz = 0.0; p = E.p_atm;
   }
   P5[0] = rho; P5[1] = vx; P5[2] = vy; P5[3] = vz; P5[4] = p;
-  if (bits) {
+  if (bits & (1 | 2 | 4 | 8)) {
     Prim P = {rho, vx, vy, vz, p, Bx, By, Bz};
     double Un[5];
     prim2con(P, M, E, Un);

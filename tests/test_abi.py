@@ -33,7 +33,7 @@ def test_header_symbols_exported(L):
 def test_struct_layouts_match_header():
     from paper_2406_11669_b200 import binding
     assert C.sizeof(binding.GrmhdOpts) == 7 * 8 + 8 * 4
-    assert C.sizeof(binding.GrmhdStats) == 5 * 8 + 6 * 8
+    assert C.sizeof(binding.GrmhdStats) == 5 * 8 + 7 * 8
 
 
 def test_workspace_bytes_and_validation(L):

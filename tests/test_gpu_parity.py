@@ -120,6 +120,51 @@ def test_con2prim_batch_matches_oracle():
     assert nbad_it <= 0.01 * cons.shape[1]
 
 
+def test_con2prim1d_batch_matches_oracle():
+    """Row F4: the 1-D scheme on the config-4b states: same status, the
+    oracle's primitives (the bracketing stops at a relative width of 1e-14; the recovery
+    amplifies that like the 2-D scheme)."""
+    import torch
+    from paper_2406_11669_b200 import binding
+    prim, met = wl.c2p_states(4099)
+    kw = dict(gamma_ad=5.0 / 3.0, rho_atm=1e-10, p_floor=1e-10, w_max=100.0)
+    og, orf = binding.make_opts(**kw), ref.make_opts(**kw)
+    cons = np.ascontiguousarray(np.stack([ref.prim2con_pt(prim[:, q], met[:, q], 5.0 / 3.0)
+                                          for q in range(prim.shape[1])], axis=1))
+    P, st, it = binding.con2prim1d_batch(torch.from_numpy(cons).cuda(),
+                                         torch.from_numpy(met).cuda(), og)
+    P, st, it = P.cpu().numpy(), st.cpu().numpy(), it.cpu().numpy()
+    worst = 0.0
+    for q in range(cons.shape[1]):
+        p, s1, _ = ref.con2prim1d_pt(cons[:, q], met[:, q], orf)
+        assert st[q] == s1 == 0, (q, st[q], s1)
+        rhoh = p[0] + 2.5 * p[4]
+        worst = max(worst, abs(P[0, q] - p[0]) / p[0], np.abs(P[1:4, q] - p[1:4]).max(),
+                    abs(P[4, q] - p[4]) / rhoh)
+    REPORT.append({"case": "con2prim1d batch", "tol": 1e-10, "max": float(worst)})
+    assert worst <= 1e-10, worst
+    assert it.max() <= 60
+
+
+def test_backup_con2prim_in_the_step():
+    """Option c2p_backup on both sides with a Newton budget too small to converge: the 1-D
+    scheme recovers the cells the 2-D scheme gives up on; same counters, same state."""
+    w = wl.c2p_stress(24)
+    w2 = wl.Workload(**{**w.__dict__, "opts": {**w.opts, "c2p_maxit": 3},
+                        "name": w.name + "_backup"})
+    r, g = make_ref(w2), make_gpu(w2)
+    r.set_option("c2p_backup", 1.0)
+    g.set_option("c2p_backup", 1.0)
+    r.step(1, w2.cfl)
+    g.step(1, w2.cfl)
+    _assert_cons(to_np(g.get_cons()), r.get_cons(), 1e-10, w2.name)
+    sg, sr = g.stats(), r.stats()
+    assert sr["c2p_backup"] > 100
+    assert abs(sg["c2p_backup"] - sr["c2p_backup"]) <= 0.01 * sr["c2p_backup"]
+    assert sg["c2p_fail"] == sr["c2p_fail"]
+    g.close()
+
+
 # ------------------------------------------------------------------ one step, all configs
 def test_config1_balsara_one_step():
     _one_step_case(wl.balsara1(256, 4, 4))
