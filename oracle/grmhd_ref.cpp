@@ -13,7 +13,7 @@
 // P6 curl/div/flux-CT identities, P7 HLLE consistency, P8 reconstruction properties,
 // P9 speeds closed forms, P10 con2prim closed forms, P11 sources vs brute-force 4-D
 // Christoffels, P12 naive re-evaluation on 4^3 blocks, P13 constant-metric advection,
-// P14 Rindler hydrostatic equilibrium.  Parity UNPINNED by the paper: the PPM variant (G8)
+// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45).  Parity UNPINNED by the paper: the PPM variant (G8)
 // and the characteristic-speed bound (G9) are readings of citations that are not in
 // PAPER.md; they are pinned only by the mathematical properties P8/P9.
 #include "grmhd_ref.h"
