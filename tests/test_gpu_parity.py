@@ -205,6 +205,28 @@ def test_tiny_and_degenerate_blocks():
     _one_step_case(wl.balsara1(8, 2, 2), nsteps=2)
 
 
+def _crop(w, nx, ny, nz, name):
+    """Lower corner (nx, ny, nz) of an outflow workload: arrays are [z][y][x] incl. 3 ghosts
+    (staggered ones one longer)."""
+    cc = (slice(0, nz + 6), slice(0, ny + 6), slice(0, nx + 6))
+    st = (slice(0, nz + 7), slice(0, ny + 7), slice(0, nx + 7))
+    cut = lambda a, sl: None if a is None else np.ascontiguousarray(a[sl])
+    return wl.Workload(name=name, nx=nx, ny=ny, nz=nz, dx=w.dx, opts=dict(w.opts),
+                       metric=[cut(a, cc) for a in w.metric], prims=[cut(a, cc) for a in w.prims],
+                       vecpot=None if w.vecpot is None else [cut(a, st) for a in w.vecpot],
+                       mask=cut(w.mask, cc), cfl=w.cfl)
+
+
+def test_odd_and_non_cubic_blocks():
+    """Extents that are not multiples of 4 or 32, different per axis, around the 32-wide groups
+    of the TMA kernel and the 27-face segments of the lanes-along-D kernel."""
+    w = wl.kerr_blob(72)
+    for (nx, ny, nz) in ((37, 33, 35), (65, 31, 34), (28, 55, 63)):
+        for opts in (None, {"flux_x_rows": 0.0}):
+            _one_step_case(_crop(w, nx, ny, nz, f"kerr_crop_{nx}x{ny}x{nz}"), gpu_options=opts)
+    _one_step_case(wl.c2p_stress(45))     # periodic, odd
+
+
 def test_every_flux_kernel_is_covered():
     """The three implementations of A3+A4 give the oracle's result: k_flux_xrow + k_flux_tma
     (default), k_flux_tma for x as well, and the marching kernel k_flux_march everywhere."""
