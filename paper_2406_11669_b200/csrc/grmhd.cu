@@ -30,6 +30,8 @@ struct grmhd {
   int nfields = 0;
   long long stage_elems = 0;
   bool have_metric = false, have_prims = false, have_mask = false;
+  bool dirty = false;  // set_prims / set_vecpot changed the inputs: (B, U~, sources, max speed)
+                       // are rebuilt once, by the next call that needs them
   double cfl_set = -1.0, fixed_dt = 0.0, fixed_set = -1.0, tend_set = -2.0;
   long long steps = 0;
   long long launches = 0;
@@ -491,6 +493,7 @@ int one_step(grmhd* h) {
 // field_from_potential + prim->cons + max speed
 int init_state(grmhd* h) {
   const Geom& g = h->g;
+  h->dirty = false;
   int rc = fill_ghosts(h, fill_vecpot());
   if (rc) return rc;
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 0);
@@ -613,7 +616,8 @@ int grmhd_set_prims(grmhd* h, const double* const field[8]) {
   h->steps = 0;
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 1);
   CKL("k_reset_state");
-  return init_state(h);
+  h->dirty = true;
+  return GRMHD_OK;
 }
 
 int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
@@ -626,7 +630,8 @@ int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
     int rc = copy_in(h, field[d], F_Y + 5 + d, true);
     if (rc) return rc;
   }
-  return init_state(h);
+  h->dirty = true;
+  return GRMHD_OK;
 }
 
 int grmhd_set_mask(grmhd* h, const unsigned char* mask) {
@@ -649,8 +654,9 @@ int grmhd_step(grmhd* h, int n, double cfl) {
   if (!h) return GRMHD_EINVAL;
   if (n < 0) return fail(h, GRMHD_EINVAL, "step: n < 0");
   if (!h->have_metric || !h->have_prims) return fail(h, GRMHD_ESTATE, "step before set_metric/set_prims");
-  int rc = set_params(h, cfl, -1.0);
+  int rc = h->dirty ? init_state(h) : GRMHD_OK;
   if (rc) return rc;
+  if ((rc = set_params(h, cfl, -1.0))) return rc;
   for (int s = 0; s < n; s++)
     if ((rc = one_step(h))) return rc;
   return GRMHD_OK;
@@ -660,7 +666,9 @@ int grmhd_step_until(grmhd* h, double t_end, double cfl, int* nsteps_done) {
   if (!h) return GRMHD_EINVAL;
   if (!h->have_metric || !h->have_prims) return fail(h, GRMHD_ESTATE, "step_until before set_metric/set_prims");
   if (t_end < 0) return fail(h, GRMHD_EINVAL, "step_until: t_end < 0");
-  int rc = set_params(h, cfl, t_end);
+  int rc = h->dirty ? init_state(h) : GRMHD_OK;
+  if (rc) return rc;
+  rc = set_params(h, cfl, t_end);
   if (rc) return rc;
   int n = 0;
   for (;;) {
@@ -679,6 +687,7 @@ int grmhd_step_until(grmhd* h, double t_end, double cfl, int* nsteps_done) {
 int grmhd_get_prims(grmhd* h, double* const field[8]) {
   if (!h) return GRMHD_EINVAL;
   if (!field) return fail(h, GRMHD_EINVAL, "get_prims: NULL field array");
+  if (h->dirty) { int rc0 = init_state(h); if (rc0) return rc0; }
   for (int r = 0; r < 8; r++) {
     if (!field[r]) return fail(h, GRMHD_EINVAL, "get_prims: NULL field");
     int rc = copy_out(h, r < 5 ? F_P + r : F_BC + (r - 5), field[r], false, 0);
@@ -691,6 +700,7 @@ int grmhd_get_prims(grmhd* h, double* const field[8]) {
 int grmhd_get_cons(grmhd* h, double* const field[8]) {
   if (!h) return GRMHD_EINVAL;
   if (!field) return fail(h, GRMHD_EINVAL, "get_cons: NULL field array");
+  if (h->dirty) { int rc0 = init_state(h); if (rc0) return rc0; }
   for (int r = 0; r < 8; r++) {
     if (!field[r]) return fail(h, GRMHD_EINVAL, "get_cons: NULL field");
     int rc = copy_out(h, r < 5 ? F_Y + r : F_BC + (r - 5), field[r], false, r < 5 ? 1 : 2);
@@ -703,6 +713,7 @@ int grmhd_get_cons(grmhd* h, double* const field[8]) {
 int grmhd_get_vecpot(grmhd* h, double* const field[3]) {
   if (!h) return GRMHD_EINVAL;
   if (!field) return fail(h, GRMHD_EINVAL, "get_vecpot: NULL field array");
+  if (h->dirty) { int rc0 = init_state(h); if (rc0) return rc0; }
   for (int d = 0; d < 3; d++) {
     if (!field[d]) return fail(h, GRMHD_EINVAL, "get_vecpot: NULL field");
     int rc = copy_out(h, F_Y + 5 + d, field[d], true, 0);
@@ -750,6 +761,7 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
 
 int grmhd_get_stats(grmhd* h, grmhd_stats* out) {
   if (!h || !out) return GRMHD_EINVAL;
+  if (h->dirty) { int rc0 = init_state(h); if (rc0) return rc0; }
   DevState st;
   CK(cudaMemcpyAsync(&st, h->dst, sizeof st, cudaMemcpyDeviceToHost, h->s));
   CK(cudaStreamSynchronize(h->s));
