@@ -13,7 +13,7 @@
 // P6 curl/div/flux-CT identities, P7 HLLE consistency, P8 reconstruction properties,
 // P9 speeds closed forms, P10 con2prim closed forms, P11 sources vs brute-force 4-D
 // Christoffels, P12 naive re-evaluation on 4^3 blocks, P13 constant-metric advection,
-// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45).  Parity UNPINNED by the paper: the PPM variant (G8)
+// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45), P16 upwind CT (eqs 33-35).  Parity UNPINNED by the paper: the PPM variant (G8)
 // and the characteristic-speed bound (G9) are readings of citations that are not in
 // PAPER.md; they are pinned only by the mathematical properties P8/P9.
 #include "grmhd_ref.h"
@@ -168,8 +168,12 @@ void face_floors(double P[8], const Metric& M, const ref_opts& o) {
 // R7: HLLE eq. (29) PAPER.md:196 (riemann = 0) or LxF eq. (30) PAPER.md:203 (riemann = 1).
 // G10: the flux paired with the coordinate speeds is G = alpha_f F^d.  Returns F^ (not yet
 // multiplied by sqrt(gamma_f)).
+// `uct` (optional, 4 values): what the upwind constrained transport of PAPER.md:229-250 needs
+// from this face -- a_+ and a_- of eq. (34) and the upwind transverse velocities of eq. (33),
+// vbar^j = (a_+ v~^jL + a_- v~^jR)/(a_+ + a_-) for j = (d+1)%3, (d+2)%3 (their mean when
+// a_+ + a_- vanishes), v~^j = alpha v^j - beta^j with the face metric.
 void riemann(int d, const double PL_in[8], const double PR_in[8], const Metric& M,
-             const ref_opts& o, double Fhat[8]) {
+             const ref_opts& o, double Fhat[8], double* uct = nullptr) {
   double PL[8], PR[8];
   std::memcpy(PL, PL_in, sizeof PL);
   std::memcpy(PR, PR_in, sizeof PR);
@@ -198,6 +202,22 @@ void riemann(int d, const double PL_in[8], const double PR_in[8], const Metric& 
     }
   }
   Fhat[5 + d] = 0.0;  // the B^d row of eq. (18) vanishes identically
+  if (uct) {
+    uct[0] = cmax;  // eq. (34): a_+ = max{0, lambda_+(U^L), lambda_+(U^R)}
+    uct[1] = cmin;  //           a_- = max{0, -lambda_-(U^L), -lambda_-(U^R)}
+    for (int t = 0; t < 2; t++) {
+      const int j = (d + 1 + t) % 3;
+      const double vL = M.alpha * PL[1 + j] - M.beta[j], vR = M.alpha * PR[1 + j] - M.beta[j];
+      uct[2 + t] = cmax + cmin < 1e-300 ? 0.5 * (vL + vR)
+                                        : (cmax * vL + cmin * vR) / (cmax + cmin);  // eq. (33)
+    }
+  }
+}
+
+// eq. (35), one bracket: [a_+ v^L B^L + a_- v^R B^R - a_+ a_- (B^R - B^L)]/(a_+ + a_-)
+inline double uct_bracket(double ap, double am, double vL, double vR, double BL, double BR) {
+  if (ap + am < 1e-300) return 0.5 * (vL * BL + vR * BR);
+  return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) / (ap + am);
 }
 
 // ---------------------------------------------------------------------- reconstruction
@@ -608,6 +628,8 @@ struct ref_grmhd {
   std::vector<double> U[5];    // densitised D~, S~_j, tau~
   std::vector<double> A[3];    // vector potential on edges
   std::vector<double> F[3][8]; // stored fluxes
+  std::vector<double> W[3][4]; // UCT face data per direction: a_+, a_-, vbar^{(d+1)%3}, vbar^{(d+2)%3}
+  int emf = 0;                 // option "emf": 0 flux-CT (R10), 1 upwind CT
   std::vector<uint8_t> mask;
   bool have_metric = false, have_prims = false, have_mask = false;
   double t = 0, dt = 0, fixed_dt = 0, maxspeed[3] = {0, 0, 0};
@@ -808,9 +830,14 @@ struct ref_grmhd {
     for (int d = 0; d < 3; d++) {
       const int e[3] = {d == 0, d == 1, d == 2};
       for (int r = 0; r < 8; r++) std::fill(F[d][r].begin(), F[d][r].end(), 0.0);
-      // faces f = 0..n_d along d; transverse cells with a 1-cell apron (R10)
-      const int lo[3] = {e[0] ? 0 : -1, e[1] ? 0 : -1, e[2] ? 0 : -1};
-      const int hi[3] = {e[0] ? nx : nx, e[1] ? ny : ny, e[2] ? nz : nz};  // inclusive
+      // faces f = 0..n_d along d; transverse cells with a 1-cell apron (R10), or with the 3
+      // cells the face -> edge PPM stencils of the upwind CT reach (G26)
+      const int ap = emf == 1 ? 3 : 1;
+      if (emf == 1)
+        for (int r = 0; r < 4; r++) W[d][r].assign(NP, 0.0);
+      const int lo[3] = {e[0] ? 0 : -ap, e[1] ? 0 : -ap, e[2] ? 0 : -ap};
+      const int hi[3] = {e[0] ? nx : nx + ap - 1, e[1] ? ny : ny + ap - 1,
+                         e[2] ? nz : nz + ap - 1};  // inclusive
 #pragma omp parallel for num_threads(g_threads)
       for (int k = lo[2]; k <= hi[2]; k++)
         for (int j = lo[1]; j <= hi[1]; j++)
@@ -827,8 +854,11 @@ struct ref_grmhd {
             recon_face(d, c, o, PL, PR);
             // G6: the normal component is the single-valued staggered field
             PL[5 + d] = PR[5 + d] = Bf[d][idx(i, j, k)] / sgf;
-            riemann(d, PL, PR, Mf, o, Fh);
+            double uct[4];
+            riemann(d, PL, PR, Mf, o, Fh, emf == 1 ? uct : nullptr);
             for (int r = 0; r < 8; r++) F[d][r][idx(i, j, k)] = sgf * Fh[r];
+            if (emf == 1)
+              for (int r = 0; r < 4; r++) W[d][r][idx(i, j, k)] = uct[r];
           }
     }
   }
@@ -883,6 +913,7 @@ struct ref_grmhd {
             kU[r][c] = -div + M.alpha * sg * S[r];
           }
         }
+    if (emf == 1) { uct_rhs(kA); return; }
     // R10: flux-CT electric field on edges; R11: d_t A_i = -E_i (algebraic gauge)
     const std::vector<double>&FxBy = F[0][6], &FxBz = F[0][7], &FyBx = F[1][5],
                              &FyBz = F[1][7], &FzBx = F[2][5], &FzBy = F[2][6];
@@ -905,6 +936,46 @@ struct ref_grmhd {
                                       FyBx[idx(i - 1, j, k)] + FyBx[c]);
             kA[2][c] = -Ez;
           }
+        }
+  }
+
+  // ------------------------------------- upwind constrained transport (row F1, G26-G28)
+  // PAPER.md:229-250, eqs (33)-(35).  For the edge component E_c with (a, b, c) cyclic:
+  //   E_c = - [a-bracket of vbar^a B~^b] + [b-bracket of vbar^b B~^a]
+  // The a-bracket takes vbar^a (eq. 33, stored on the b-faces) and the staggered B~^b (on the
+  // b-faces), both reconstructed ALONG a to the edge with the PPM of G8 (no flattening): L
+  // from the lower, R from the upper side; its a_+-, a_-^a are the larger of the values on the
+  // two a-faces that share the edge.  Lower convention: edge (i,j,k) of E_z = (i-1/2, j-1/2, k).
+  double edge_bracket(int a, int b, int i, int j, int k) const {
+    const int ea[3] = {a == 0, a == 1, a == 2}, eb[3] = {b == 0, b == 1, b == 2};
+    // vbar^a on b-faces: slot 2 if a == (b+1)%3 else slot 3
+    const std::vector<double>& vb = W[b][a == (b + 1) % 3 ? 2 : 3];
+    double sv[6], sB[6];
+    for (int m = 0; m < 6; m++) {
+      const size_t c = idx(i + (m - 3) * ea[0], j + (m - 3) * ea[1], k + (m - 3) * ea[2]);
+      sv[m] = vb[c];
+      sB[m] = Bf[b][c];
+    }
+    double vL, vR, BL, BR, dum;
+    ppm_cell(sv, 0.0, dum, vL);      // q^+ of the lower cell
+    ppm_cell(sv + 1, 0.0, vR, dum);  // q^- of the upper cell
+    ppm_cell(sB, 0.0, dum, BL);
+    ppm_cell(sB + 1, 0.0, BR, dum);
+    const size_t c0 = idx(i, j, k), cm = idx(i - eb[0], j - eb[1], k - eb[2]);
+    const double ap = std::max(W[a][0][c0], W[a][0][cm]);
+    const double am = std::max(W[a][1][c0], W[a][1][cm]);
+    return uct_bracket(ap, am, vL, vR, BL, BR);
+  }
+
+  void uct_rhs(std::vector<double> kA[3]) {
+    for (int k = 0; k <= nz; k++)
+      for (int j = 0; j <= ny; j++)
+        for (int i = 0; i <= nx; i++) {
+          const size_t c = idx(i, j, k);
+          // R11: d_t A_i = -E_i
+          if (i < nx) kA[0][c] = -(-edge_bracket(1, 2, i, j, k) + edge_bracket(2, 1, i, j, k));
+          if (j < ny) kA[1][c] = -(-edge_bracket(2, 0, i, j, k) + edge_bracket(0, 2, i, j, k));
+          if (k < nz) kA[2][c] = -(-edge_bracket(0, 1, i, j, k) + edge_bracket(1, 0, i, j, k));
         }
   }
 
@@ -1207,6 +1278,7 @@ int ref_set_option(ref_grmhd* h, const char* key, double value) {
   if (!h || !key) return -1;
   if (std::strcmp(key, "fixed_dt") == 0) { h->fixed_dt = value; return 0; }
   if (std::strcmp(key, "c2p_backup") == 0) { h->c2p_backup = value != 0.0; return 0; }
+  if (std::strcmp(key, "emf") == 0) { h->emf = value != 0.0; return 0; }
   return -1;
 }
 
