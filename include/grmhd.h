@@ -137,6 +137,10 @@ int grmhd_get_cons(grmhd* h, double* const field[8]);
 int grmhd_get_vecpot(grmhd* h, double* const field[3]);
 
 /* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off);
+ * "emf" (0 default: electric field on the edges by flux-CT, R10; 1: upwind constrained
+ * transport, eqs (33)-(35) PAPER.md:229-250 -- the flux kernels then also store a_+, a_- and the
+ * upwind transverse velocities of every face on a 3-cell transverse apron, and the edges are
+ * updated by their own kernel);
  * "c2p_backup" (1: when the 2-D Newton con2prim fails, try the 1-D scheme of PAPER.md:297-320,
  * eqs (42)-(45), before resetting the cell to atmosphere -- the paper's policy, PAPER.md:684;
  * 0 = off, the default: failure -> atmosphere, G20);

@@ -193,7 +193,7 @@ template <int D>
 __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double vz, double p,
                                         double Bx, double By, double Bz, const Met& M,
                                         double gdd, const Eos& E, double U[7], double Gf[7],
-                                        double& lm, double& lp) {
+                                        double& lm, double& lp, double* vt = nullptr) {
   rho = rho < E.rho_atm ? E.rho_atm : rho;
   p = p < E.p_floor ? E.p_floor : p;
   double vlx, vly, vlz;
@@ -241,6 +241,7 @@ __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double
   const double B2t = D == 0 ? Bz : (D == 1 ? Bx : By);
   const double vt1 = D == 0 ? vty : (D == 1 ? vtz : vtx);
   const double vt2 = D == 0 ? vtz : (D == 1 ? vtx : vty);
+  if (vt) { vt[0] = vt1; vt[1] = vt2; }  // v~^{(D+1)%3}, v~^{(D+2)%3} for eq. (33)
   U[5] = B1; U[6] = B2t;
   Gf[5] = B1 * vtd - Bd * vt1;
   Gf[6] = B2t * vtd - Bd * vt2;
@@ -263,9 +264,10 @@ __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double
 __device__ __forceinline__ void ft_hll(const double UL[7], const double GL[7], double lmL,
                                        double lpL, const double UR[7], const double GR[7],
                                        double lmR, double lpR, double sgf, int riemann,
-                                       double out[7]) {
+                                       double out[7], double* apm = nullptr) {
   const double cmax = ft_max(0.0, ft_max(lpL, lpR));
   const double cmin = -ft_min(0.0, ft_min(lmL, lmR));
+  if (apm) { apm[0] = cmax; apm[1] = cmin; }  // a_+, a_- of eq. (34)
   const double cs = cmax + cmin;
   if (riemann == 1) {  // eq. (30)
     const double cw = ft_max(cmax, cmin);
@@ -283,6 +285,21 @@ __device__ __forceinline__ void ft_hll(const double UL[7], const double GL[7], d
   }
 }
 
+// Upwind-CT face data of direction D (row F1): a_+, a_- and eq. (33)
+// vbar^j = (a_+ v~^jL + a_- v~^jR)/(a_+ + a_-), their mean when a_+ + a_- vanishes.
+// o = address of this face in field F_W + 4 D.
+__device__ __forceinline__ void ft_store_uct(double* o, size_t NPA, const double apm[2],
+                                             const double vtL[2], const double vtR[2]) {
+  const double cs = apm[0] + apm[1];
+  const bool deg = cs < 1e-300;
+  const double w = ft_rcp(deg ? 1.0 : cs);
+  const double a = deg ? 0.5 : apm[0] * w, b = deg ? 0.5 : apm[1] * w;
+  o[0] = apm[0];
+  o[NPA] = apm[1];
+  o[2 * NPA] = a * vtL[0] + b * vtR[0];
+  o[3 * NPA] = a * vtL[1] + b * vtR[1];
+}
+
 // 32-byte global load of 4 consecutive doubles (address 32-byte aligned)
 __device__ __forceinline__ void ft_ld4(const double* p, double& a, double& b, double& c,
                                        double& d) {
@@ -295,9 +312,11 @@ __device__ __forceinline__ void ft_ld4(const double* p, double& a, double& b, do
 // grid: x = (groups of 32 along t0) * (n_t1 + 2), y = segments of `seglen` faces (seglen a
 // multiple of 4).  For D = 0 the march starts at face -2 so that every 4-cell group of a row
 // is one 32-byte sector.
-template <int D, int RECON>
-__global__ void __launch_bounds__(FT_THREADS, FT_MINB)
-k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
+// UCT (compile time, so that the default kernel keeps its register budget): also store the
+// upwind-CT face rows of F_W.
+template <int D, int RECON, bool UCT>
+__global__ void __launch_bounds__(FT_THREADS, UCT ? 2 : FT_MINB)
+k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx, int ap,
            const __grid_constant__ CUtensorMap tmMet, const __grid_constant__ CUtensorMap tmBf) {
   using Smem = FtSmem<D>;
   constexpr int TC = FT_TC;
@@ -310,7 +329,7 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
   const int nt0 = D == 0 ? g.ny : g.nx;
   const int sd = D == 0 ? 1 : (D == 1 ? (int)g.sy : (int)g.sz);
   const int gx = (int)blockIdx.x % ngx;
-  const int t1 = (int)blockIdx.x / ngx - 1;
+  const int t1 = (int)blockIdx.x / ngx - ap;  // ap = transverse apron: 1 (flux-CT), 3 (UCT)
   const int g0 = gx * 32;
   const int fbeg = D == 0 ? -2 : 0;
   const int f0 = fbeg + (int)blockIdx.y * seglen;
@@ -492,19 +511,24 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx,
         qR[v] = sm.q[buf][v][1][clB][plB];
       }
       double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR;
+      double vtL[2], vtR[2], apm[2];
       ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
                  D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]),
-                 M, gdd, E, UL, GL, lmL, lpL);
+                 M, gdd, E, UL, GL, lmL, lpL, UCT ? vtL : nullptr);
       ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
                  D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]),
-                 M, gdd, E, UR, GR, lmR, lpR);
+                 M, gdd, E, UR, GR, lmR, lpR, UCT ? vtR : nullptr);
       double out[7];
-      ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
+      ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out, UCT ? apm : nullptr);
       if (okB && f >= 0 && f < f1) {
         const int pl = D == 0 ? tid / TC : (tid & 31);
         double* o = outb + (D == 0 ? pl * (int)g.sy + f : pl + f * sd);
 #pragma unroll
         for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
+        if (UCT) {
+          constexpr int fid = D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ);
+          ft_store_uct(o + (size_t)(F_W + 4 * D - fid) * NPA, NPA, apm, vtL, vtR);
+        }
       }
     }
     // no barrier here: the next phase A writes the other exchange buffer

@@ -63,18 +63,23 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
   }
 }
 
-// grid: one warp per (pencil, segment) item.
-// D = 0: every row of the block incl. the flux-CT apron: item = row * nsd + seg,
-//        row = (k+1)*(ny+2) + (j+1).
-// D = 1, 2: only the two apron columns x = -1 and x = nx that the 32-wide groups of
-//        k_flux_tma leave out (lanes then run along y or z with a stride: uncoalesced, but
-//        it is 2 columns): item = ((t1+1) * 2 + col) * nsd + seg.
+// grid: one warp per (pencil, segment) item: item = pencil * nsd + seg.  With (t0, t1) the
+// transverse axes -- (y, z) for D = x, (x, z) for D = y, (x, y) for D = z -- and `ap` the
+// transverse apron (1 for flux-CT, R10; 3 for the upwind CT, G27):
+//   mode 0: every pencil t0 in [-ap, n_t0 + ap), t1 in [-ap, n_t1 + ap).  The x fluxes; for
+//           D = y, z the lanes then run along y or z with a stride (uncoalesced: small
+//           blocks and option combinations only).
+//   mode 1: only the 2 ap apron columns t0 < 0 and t0 >= n_t0 that the 32-wide groups of
+//           k_flux_tma leave out.
 template <int D, int RECON>
 __global__ void __launch_bounds__(FX_THREADS, FX_MINB)
-k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems) {
+k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems, int ap,
+            int mode) {
   const int lane = threadIdx.x & 31;
   const long long nwarp = (long long)gridDim.x * (FX_THREADS / 32);
   const int nD = g.n(D);
+  const int nt0 = D == 0 ? g.ny : g.nx;
+  const int w0 = mode ? 2 * ap : nt0 + 2 * ap;
   const int sd = D == 0 ? 1 : (D == 1 ? (int)g.sy : (int)g.sz);
   // grid-stride loop over the items (the launch gives every warp one item)
   for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
@@ -83,14 +88,9 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems)
   const int row = (int)(item / nsd);
   const int c = seg * FX_VALID - 3 + lane;  // this lane's cell along D; its face is c - 1/2
   const int cc = min(c, nD + G - 1);        // lanes past the last ghost cell reuse it
-  int idx;
-  if (D == 0) {
-    idx = (int)g.at(cc, row % (g.ny + 2) - 1, row / (g.ny + 2) - 1);
-  } else {
-    const int xc = (row & 1) ? g.nx : -1;
-    const int t1 = (row >> 1) - 1;
-    idx = (int)(D == 1 ? g.at(xc, cc, t1) : g.at(xc, t1, cc));
-  }
+  const int q0 = row % w0, t1 = row / w0 - ap;
+  const int t0 = mode ? (q0 < ap ? q0 - ap : nt0 + q0 - ap) : q0 - ap;
+  const int idx = (int)(D == 0 ? g.at(cc, t0, t1) : (D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc)));
 
   // ---- cell data of the lane: rho, v^x, v^y, v^z, p, B^y, B^z
   double q[FM_NV];
@@ -145,21 +145,22 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems)
   const double sgf = det * isg;
   const double gdd = inv_gamma_dd<D>(M, isg * isg);
   const double Bn = bfx * isg;  // G6
-  double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR;
+  double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR, vtL[2], vtR[2], apm[2];
   // slots 5, 6 hold B^{(D+1)%3}, B^{(D+2)%3}
   ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
              D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]), M,
-             gdd, E, UL, GL, lmL, lpL);
+             gdd, E, UL, GL, lmL, lpL, vtL);
   ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
              D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]), M,
-             gdd, E, UR, GR, lmR, lpR);
+             gdd, E, UR, GR, lmR, lpR, vtR);
   double out[7];
-  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out);
+  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out, apm);
   if (lane >= 3 && lane < 3 + FX_VALID && c <= nD) {
     double* o = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
     for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
+    if (E.emf) ft_store_uct(fld(base, g, F_W + 4 * D) + idx, NPA, apm, vtL, vtR);
   }
   }  // items
 }

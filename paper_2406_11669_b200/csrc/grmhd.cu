@@ -36,7 +36,7 @@ struct grmhd {
   long long steps = 0;
   long long launches = 0;
   int fm_conc[9] = {0};  // resident blocks of each flux-kernel instantiation (0 = not queried)
-  int ft_conc[9] = {0};  // ... of the TMA-fed instantiations
+  int ft_conc[18] = {0};  // ... of the TMA-fed instantiations
   CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][.] of the ring stages, per direction
   bool tma_ok = false;
   int xrow = 1;          // x fluxes: 1 k_flux_xrow (lanes along x), 0 as y and z
@@ -143,6 +143,7 @@ Eos make_eos(const grmhd_opts& o) {
   E.flatten = o.ppm_flatten;
   E.riemann = o.riemann;
   E.c2p_backup = 0;
+  E.emf = 0;
   return E;
 }
 
@@ -330,17 +331,22 @@ int launch_flux(grmhd* h, int apron) {
   return GRMHD_OK;
 }
 
-// lanes along D (flux_xrow.cuh): one warp per 27 faces of a pencil.  D = 0: every row;
-// D = 1, 2: the two apron columns of k_flux_tma.
+// lanes along D (flux_xrow.cuh): one warp per 27 faces of a pencil.  mode 0: every pencil
+// (the x fluxes; any direction of a narrow block when the upwind CT is on); mode 1: the
+// apron columns k_flux_tma leaves out.
+int apron_width(const grmhd* h) { return h->E.emf ? 3 : 1; }  // G27: PPM face -> edge stencils
+
 template <int D, int RECON>
-int launch_flux_xrow(grmhd* h) {
+int launch_flux_xrow(grmhd* h, int mode) {
   const Geom& g = h->g;
+  const int ap = apron_width(h);
   const int nsd = (g.n(D) + 1 + FX_VALID - 1) / FX_VALID;
-  const long long npen = D == 0 ? (long long)(g.ny + 2) * (g.nz + 2)
-                                : 2LL * ((D == 2 ? g.ny : g.nz) + 2);
+  const int nt0 = D == 0 ? g.ny : g.nx, nt1 = D == 2 ? g.ny : g.nz;
+  const long long npen = (long long)(mode ? 2 * ap : nt0 + 2 * ap) * (nt1 + 2 * ap);
   const long long nitems = npen * nsd;
   const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
-  k_flux_xrow<D, RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd, nitems);
+  k_flux_xrow<D, RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd, nitems,
+                                                                ap, mode);
   h->launches++;
   return GRMHD_OK;
 }
@@ -387,12 +393,12 @@ bool make_tensor_maps(grmhd* h) {
   return true;
 }
 
-template <int D, int RECON>
-int launch_flux_tma(grmhd* h) {
+template <int D, int RECON, bool UCT>
+int launch_flux_tma_v(grmhd* h) {
   const Geom& g = h->g;
-  auto kern = k_flux_tma<D, RECON>;
+  auto kern = k_flux_tma<D, RECON, UCT>;
   const int smem = (int)sizeof(FtSmem<D>);
-  const int cfg = D * 3 + RECON;
+  const int cfg = (UCT ? 9 : 0) + D * 3 + RECON;
   if (h->ft_conc[cfg] == 0) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int nb = 0, dev = 0, nsm = 0;
@@ -403,7 +409,8 @@ int launch_flux_tma(grmhd* h) {
   }
   const int nt0 = D == 0 ? g.ny : g.nx, nt1 = D == 2 ? g.ny : g.nz;
   const int ngx = (nt0 + 31) / 32;
-  const long long ngroups = (long long)ngx * (nt1 + 2);
+  const int ap = apron_width(h);
+  const long long ngroups = (long long)ngx * (nt1 + 2 * ap);
   const int nfaces = g.n(D) + 1 + (D == 0 ? 2 : 0);  // D = x marches from face -2 (alignment)
   int best = 1;
   double best_cost = 1e300;
@@ -419,13 +426,18 @@ int launch_flux_tma(grmhd* h) {
   const int seglen = ((nfaces + best - 1) / best + FT_TC - 1) / FT_TC * FT_TC;
   const int nseg = (nfaces + seglen - 1) / seglen;
   kern<<<dim3((unsigned)ngroups, nseg), FT_THREADS, smem, h->s>>>(h->base, g, h->E, seglen, ngx,
-                                                                  h->tm_met[D], h->tm_bf[D]);
+                                                                  ap, h->tm_met[D], h->tm_bf[D]);
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_tma");
-  // the two apron columns along t0
-  if (D != 0 && h->xrow) return launch_flux_xrow<D, RECON>(h);
+  // the apron columns along t0 (the marching kernel only knows the 1-cell apron)
+  if ((D != 0 && h->xrow) || h->E.emf) return launch_flux_xrow<D, RECON>(h, 1);
   return launch_flux<D, RECON>(h, 1);
+}
+
+template <int D, int RECON>
+int launch_flux_tma(grmhd* h) {
+  return h->E.emf ? launch_flux_tma_v<D, RECON, true>(h) : launch_flux_tma_v<D, RECON, false>(h);
 }
 
 template <int D>
@@ -434,11 +446,14 @@ int launch_flux_d(grmhd* h) {
   const int nt0 = D == 0 ? h->g.ny : h->g.nx;
   int rc;
   if (D == 0 && h->flux_impl == 1 && h->xrow)
-    rc = recon == 0 ? launch_flux_xrow<0, 0>(h)
-                    : (recon == 1 ? launch_flux_xrow<0, 1>(h) : launch_flux_xrow<0, 2>(h));
+    rc = recon == 0 ? launch_flux_xrow<0, 0>(h, 0)
+                    : (recon == 1 ? launch_flux_xrow<0, 1>(h, 0) : launch_flux_xrow<0, 2>(h, 0));
   else if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
     rc = recon == 0 ? launch_flux_tma<D, 0>(h)
                     : (recon == 1 ? launch_flux_tma<D, 1>(h) : launch_flux_tma<D, 2>(h));
+  else if (h->E.emf)  // the marching kernel has neither the 3-cell apron nor the UCT face rows
+    rc = recon == 0 ? launch_flux_xrow<D, 0>(h, 0)
+                    : (recon == 1 ? launch_flux_xrow<D, 1>(h, 0) : launch_flux_xrow<D, 2>(h, 0));
   else
     rc = recon == 0 ? launch_flux<D, 0>(h, 0)
                     : (recon == 1 ? launch_flux<D, 1>(h, 0) : launch_flux<D, 2>(h, 0));
@@ -475,9 +490,15 @@ int one_step(grmhd* h) {
     int rc = compute_fluxes(h);
     if (rc) return rc;
     KT(KG_UPDATE, {
-      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 8 * (g.nz + 1)), dim3(128, 2, 1), 0,
-                 h->s>>>(h->base, g, h->dst, st[s]);
+      const int nrows = h->E.emf ? 5 : 8;  // with the upwind CT the edges have their own kernel
+      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, nrows * (g.nz + 1)),
+                 dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], nrows);
       CKL("k_update");
+      if (h->E.emf) {
+        k_emf_uct<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 3 * (g.nz + 1)),
+                    dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s]);
+        CKL("k_emf_uct");
+      }
     });
     rc = after_stage(h, s == ns - 1);
     if (rc) return rc;
@@ -732,6 +753,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "flux_kernel") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
     h->flux_impl = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "emf") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: emf is 0 or 1");
+    h->E.emf = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "c2p_backup") == 0) {

@@ -46,9 +46,11 @@ enum FieldId {
   F_FY = 53,    // 7 : y-fluxes (+ B^z, B^x rows)
   F_FZ = 60,    // 7 : z-fluxes (+ B^x, B^y rows)
   F_SRC = 67,   // 4 : alpha sqrt(gamma) S of eq. (19) for the rows S_x, S_y, S_z, tau (cells)
-  F_KS = 71,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
-  F_END_RK23 = 71,
-  F_END_RK4 = 79
+  F_W = 71,     // 12: upwind-CT face data, 4 per direction d: a_+, a_- (eq. 34) and the upwind
+                //     transverse velocities vbar^{(d+1)%3}, vbar^{(d+2)%3} (eq. 33); F_W + 4 d + r
+  F_KS = 83,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
+  F_END_RK23 = 83,
+  F_END_RK4 = 91
 };
 
 // device-resident scalars of a handle

@@ -165,6 +165,30 @@ def test_backup_con2prim_in_the_step():
     g.close()
 
 
+def test_upwind_ct_matches_oracle():
+    """Row F1: E on the edges by the upwind constrained transport (eqs 33-35) on both sides;
+    wide blocks (TMA kernels with the 3-cell apron), a narrow one (lanes-along-D kernel in every
+    direction), minmod, RK4, and the x fluxes through the TMA kernel."""
+    cases = [(wl.kerr_blob(40), None), (wl.blast(44), None), (wl.c2p_stress(36), None),
+             (wl.bns_like(32), None), (wl.kerr_blob(40), {"flux_x_rows": 0.0}),
+             (wl.alfven_wave(16, 1, 1, axis=0), None), (wl.balsara1(64, 4, 4), None)]
+    for w, extra in cases:
+        r, g = make_ref(w), make_gpu(w)
+        r.set_option("emf", 1.0)
+        g.set_option("emf", 1.0)
+        for key, val in (extra or {}).items():
+            g.set_option(key, val)
+        nsteps = 1 if "c2p_stress" in w.name else 2   # the stress field is at the edge of the
+        r.step(nsteps, w.cfl)                         # recovery's domain after one step
+        g.step(nsteps, w.cfl)
+        _assert_cons(to_np(g.get_cons()), r.get_cons(), 10 * TOL1, w.name + " uct")
+        Ag, Ar = to_np(g.get_vecpot()), r.get_vecpot()
+        amax = max(max(np.abs(a).max() for a in Ar), 1e-300)
+        for d in range(3):
+            assert np.abs(Ag[d] - Ar[d]).max() / amax <= 10 * TOL1, (w.name, "A", d)
+        g.close()
+
+
 # ------------------------------------------------------------------ one step, all configs
 def test_config1_balsara_one_step():
     _one_step_case(wl.balsara1(256, 4, 4))
