@@ -14,6 +14,7 @@
 #include "flux_march.cuh"
 #include "flux_tma.cuh"
 #include "flux_xrow.cuh"
+#include "emf_uct.cuh"
 #include "kernels_batch.cuh"
 
 using namespace gk;

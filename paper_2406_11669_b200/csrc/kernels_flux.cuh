@@ -152,49 +152,4 @@ k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkS
   rk_apply(base, g, r, c, rhs, h, rk);
 }
 
-// ---------------------------------------------------------- upwind constrained transport
-// Row F1, eqs (33)-(35), readings G26-G28 of DESIGN.md.  One bracket of
-// eq. (35): the quantities on the b-faces -- vbar^a (eq. 33, stored by the b-direction flux
-// kernel in F_W) and the staggered B~^b -- reconstructed along a to the edge (PPM of G8, no
-// flattening: L from the lower, R from the upper side), combined with the larger a_+, a_- of
-// the two a-faces that share the edge.  c = index of the edge, sa / sb = strides of a and b.
-__device__ __forceinline__ double uct_bracket(const double* __restrict__ base, const Geom& g,
-                                              int a, int b, long long c, long long sa,
-                                              long long sb) {
-  const double* vb = fld(base, g, F_W + 4 * b + (a == (b + 1) % 3 ? 2 : 3));
-  const double* Bb = fld(base, g, F_BF + b);
-  double sv[6], sB[6];
-#pragma unroll
-  for (int m = 0; m < 6; m++) {
-    sv[m] = vb[c + (m - 3) * sa];
-    sB[m] = Bb[c + (m - 3) * sa];
-  }
-  double vL, vR, BL, BR;
-  recon_pair(1, sv, 0.0, 0.0, vL, vR);
-  recon_pair(1, sB, 0.0, 0.0, BL, BR);
-  const double* Ap = fld(base, g, F_W + 4 * a);
-  const double* Am = fld(base, g, F_W + 4 * a + 1);
-  const double ap = fmax(Ap[c], Ap[c - sb]);
-  const double am = fmax(Am[c], Am[c - sb]);
-  if (ap + am < 1e-300) return 0.5 * (vL * BL + vR * BR);
-  return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) / (ap + am);
-}
-
-// One thread per edge: blockIdx.z = 3 k + comp; E_comp = -[a-bracket] + [b-bracket] with
-// (a, b, comp) cyclic, then R11 d_t A_comp = -E_comp and the RK combination.
-__global__ void __launch_bounds__(256)
-k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z / 3;
-  const int comp = blockIdx.z % 3;
-  if (i > g.nx || j > g.ny) return;
-  if ((comp == 0 && i >= g.nx) || (comp == 1 && j >= g.ny) || (comp == 2 && k >= g.nz)) return;
-  const long long c = g.at(i, j, k);
-  const int a = (comp + 1) % 3, b = (comp + 2) % 3;
-  const long long sa = g.stride(a), sb = g.stride(b);
-  const double E = -uct_bracket(base, g, a, b, c, sa, sb) + uct_bracket(base, g, b, a, c, sb, sa);
-  rk_apply(base, g, 5 + comp, c, -E, st->dt, rk);
-}
-
 }  // namespace gk
