@@ -13,7 +13,7 @@
 // P6 curl/div/flux-CT identities, P7 HLLE consistency, P8 reconstruction properties,
 // P9 speeds closed forms, P10 con2prim closed forms, P11 sources vs brute-force 4-D
 // Christoffels, P12 naive re-evaluation on 4^3 blocks, P13 constant-metric advection,
-// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45), P16 upwind CT (eqs 33-35).  Parity UNPINNED by the paper: the PPM variant (G8)
+// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45), P16 upwind CT (eqs 33-35), P17 the generalised Lorenz gauge (eqs 31-32).  Parity UNPINNED by the paper: the PPM variant (G8)
 // and the characteristic-speed bound (G9) are readings of citations that are not in
 // PAPER.md; they are pinned only by the mathematical properties P8/P9.
 #include "grmhd_ref.h"
@@ -627,6 +627,10 @@ struct ref_grmhd {
   std::vector<double> B0[3];   // static part B~0 (G16)
   std::vector<double> U[5];    // densitised D~, S~_j, tau~
   std::vector<double> A[3];    // vector potential on edges
+  std::vector<double> Psi;     // Psi_mhd = sqrt(gamma) Phi on vertices (generalised Lorenz gauge)
+  int gauge = 0;               // option "gauge": 0 algebraic, 1 generalised Lorenz
+  double lorenz_xi = 1.5;      // option "lorenz_xi": xi = lorenz_xi / dt
+  double cur_dt = 0;           // dt of the step being taken (for xi)
   std::vector<double> F[3][8]; // stored fluxes
   std::vector<double> W[3][4]; // UCT face data per direction: a_+, a_-, vbar^{(d+1)%3}, vbar^{(d+2)%3}
   int emf = 0;                 // option "emf": 0 flux-CT (R10), 1 upwind CT
@@ -804,6 +808,10 @@ struct ref_grmhd {
 
   // everything that follows a change of (U, A): R13, R14, R15
   void after_stage() {
+    if (gauge == 1) {
+      const int sV[3] = {1, 1, 1};
+      fill_ghosts(Psi, sV, 0);  // periodic wrap / copy
+    }
     field_from_potential();
     recover_primitives();
     fill_prim_ghosts();
@@ -874,7 +882,8 @@ struct ref_grmhd {
   }
 
   // ---------------------------------------------------------- L(Y) (R8, R10, R11)
-  void rhs(std::vector<double> kU[5], std::vector<double> kA[3]) {
+  void rhs(std::vector<double> kU[5], std::vector<double> kA[3],
+           std::vector<double>* kPsi = nullptr) {
     compute_fluxes();
     for (int r = 0; r < 5; r++) kU[r].assign(NP, 0.0);
     for (int d = 0; d < 3; d++) kA[d].assign(NP, 0.0);
@@ -913,7 +922,12 @@ struct ref_grmhd {
             kU[r][c] = -div + M.alpha * sg * S[r];
           }
         }
-    if (emf == 1) { uct_rhs(kA); return; }
+    if (kPsi) kPsi->assign(NP, 0.0);
+    if (emf == 1) {
+      uct_rhs(kA);
+      if (gauge == 1 && kPsi) lorenz_terms(kA, *kPsi);
+      return;
+    }
     // R10: flux-CT electric field on edges; R11: d_t A_i = -E_i (algebraic gauge)
     const std::vector<double>&FxBy = F[0][6], &FxBz = F[0][7], &FyBx = F[1][5],
                              &FyBz = F[1][7], &FzBx = F[2][5], &FzBy = F[2][6];
@@ -936,6 +950,68 @@ struct ref_grmhd {
                                       FyBx[idx(i - 1, j, k)] + FyBx[c]);
             kA[2][c] = -Ez;
           }
+        }
+    if (gauge == 1 && kPsi) lorenz_terms(kA, *kPsi);
+  }
+
+  // ---------------------------------------- generalised Lorenz gauge (row F3, G29-G32)
+  // eqs (31), (32).  Everything is evaluated at the vertices
+  // (i-1/2, j-1/2, k-1/2) where Psi_mhd lives: the metric there is the mean of the 8 cells
+  // around the vertex (G29: the metric is cell-centred input, G3), A_j the mean of the two
+  // edges of its own axis that end at the vertex (G30).
+  struct VertexData {
+    double alpha, beta[3], sg, gu[3][3], Av[3], psi;
+  };
+  VertexData vertex(int i, int j, int k) const {
+    VertexData v;
+    Metric M;
+    double acc[10] = {0};
+    for (int c = 0; c < 8; c++) {
+      const size_t q = idx(i - (c & 1), j - ((c >> 1) & 1), k - ((c >> 2) & 1));
+      for (int f = 0; f < 10; f++) acc[f] += met[f][q];
+    }
+    for (int f = 0; f < 10; f++) acc[f] *= 0.125;
+    M = unpack_metric(acc);
+    v.alpha = M.alpha;
+    for (int a = 0; a < 3; a++) v.beta[a] = M.beta[a];
+    const double det = det3(M.g);
+    v.sg = std::sqrt(det);
+    inv3(M.g, det, v.gu);
+    v.Av[0] = 0.5 * (A[0][idx(i - 1, j, k)] + A[0][idx(i, j, k)]);
+    v.Av[1] = 0.5 * (A[1][idx(i, j - 1, k)] + A[1][idx(i, j, k)]);
+    v.Av[2] = 0.5 * (A[2][idx(i, j, k - 1)] + A[2][idx(i, j, k)]);
+    v.psi = Psi[idx(i, j, k)];
+    return v;
+  }
+  // G_A = alpha Psi/sqrt(gamma) - beta^j A_j, eq. (31) (eq. (25) prints beta^j A_i: read A_j)
+  double gauge_GA(int i, int j, int k) const {
+    const VertexData v = vertex(i, j, k);
+    return v.alpha * v.psi / v.sg - (v.beta[0] * v.Av[0] + v.beta[1] * v.Av[1] + v.beta[2] * v.Av[2]);
+  }
+  // F_Psi^d = alpha sqrt(gamma) A^d - beta^d Psi, eq. (32), A^d = gamma^{dl} A_l
+  double gauge_FPsi(int d, int i, int j, int k) const {
+    const VertexData v = vertex(i, j, k);
+    const double Au = v.gu[d][0] * v.Av[0] + v.gu[d][1] * v.Av[1] + v.gu[d][2] * v.Av[2];
+    return v.alpha * v.sg * Au - v.beta[d] * v.psi;
+  }
+  // adds -d_i G_A to d_t A_i (2-point difference of the two vertices bounding the edge, G31:
+  // a discrete gradient, so that B = curl A is untouched) and forms
+  // d_t Psi = -d_j F_Psi^j - xi alpha Psi at the vertices (2nd-order centred differences, G32)
+  void lorenz_terms(std::vector<double> kA[3], std::vector<double>& kPsi) const {
+    const double xi = cur_dt > 0 ? lorenz_xi / cur_dt : 0.0;
+    for (int k = 0; k <= nz; k++)
+      for (int j = 0; j <= ny; j++)
+        for (int i = 0; i <= nx; i++) {
+          const size_t c = idx(i, j, k);
+          const double G0 = gauge_GA(i, j, k);
+          if (i < nx) kA[0][c] -= (gauge_GA(i + 1, j, k) - G0) / dx[0];
+          if (j < ny) kA[1][c] -= (gauge_GA(i, j + 1, k) - G0) / dx[1];
+          if (k < nz) kA[2][c] -= (gauge_GA(i, j, k + 1) - G0) / dx[2];
+          double div = 0;
+          div += (gauge_FPsi(0, i + 1, j, k) - gauge_FPsi(0, i - 1, j, k)) / (2.0 * dx[0]);
+          div += (gauge_FPsi(1, i, j + 1, k) - gauge_FPsi(1, i, j - 1, k)) / (2.0 * dx[1]);
+          div += (gauge_FPsi(2, i, j, k + 1) - gauge_FPsi(2, i, j, k - 1)) / (2.0 * dx[2]);
+          kPsi[c] = -div - xi * vertex(i, j, k).alpha * Psi[c];
         }
   }
 
@@ -1018,17 +1094,18 @@ struct ref_grmhd {
   }
 
   void one_step(double h) {
-    std::vector<double> Y0[8], k1[8], k2[8], k3[8], k4[8];
-    auto Y = [&](int r) -> std::vector<double>& { return r < 5 ? U[r] : A[r - 5]; };
-    for (int r = 0; r < 8; r++) Y0[r] = Y(r);
-    auto L = [&](std::vector<double> k[8]) { rhs(k, k + 5); };
+    cur_dt = h;
+    std::vector<double> Y0[9], k1[9], k2[9], k3[9], k4[9];  // D~, S~_j, tau~, A_i, Psi_mhd
+    auto Y = [&](int r) -> std::vector<double>& { return r < 5 ? U[r] : (r < 8 ? A[r - 5] : Psi); };
+    for (int r = 0; r < 9; r++) Y0[r] = Y(r);
+    auto L = [&](std::vector<double> k[9]) { rhs(k, k + 5, &k[8]); };
     if (o.rk == 2) {
       // SSP-RK2 (Heun): Y1 = Y0 + dt L(Y0); Y^{n+1} = 1/2 Y0 + 1/2 (Y1 + dt L(Y1))
       L(k1);
-      for (int r = 0; r < 8; r++) axpby(1.0, Y0[r], h, k1[r], Y(r));
+      for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], h, k1[r], Y(r));
       after_stage();
       L(k2);
-      for (int r = 0; r < 8; r++) {
+      for (int r = 0; r < 9; r++) {
         std::vector<double>& y = Y(r);
         for (size_t q = 0; q < NP; q++) y[q] = 0.5 * Y0[r][q] + 0.5 * (y[q] + h * k2[r][q]);
       }
@@ -1036,16 +1113,16 @@ struct ref_grmhd {
     } else if (o.rk == 3) {
       // SSP-RK3 (Shu-Osher)
       L(k1);
-      for (int r = 0; r < 8; r++) axpby(1.0, Y0[r], h, k1[r], Y(r));
+      for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], h, k1[r], Y(r));
       after_stage();
       L(k2);
-      for (int r = 0; r < 8; r++) {
+      for (int r = 0; r < 9; r++) {
         std::vector<double>& y = Y(r);
         for (size_t q = 0; q < NP; q++) y[q] = 0.75 * Y0[r][q] + 0.25 * (y[q] + h * k2[r][q]);
       }
       after_stage();
       L(k3);
-      for (int r = 0; r < 8; r++) {
+      for (int r = 0; r < 9; r++) {
         std::vector<double>& y = Y(r);
         for (size_t q = 0; q < NP; q++)
           y[q] = (1.0 / 3.0) * Y0[r][q] + (2.0 / 3.0) * (y[q] + h * k3[r][q]);
@@ -1054,16 +1131,16 @@ struct ref_grmhd {
     } else {
       // classic RK4
       L(k1);
-      for (int r = 0; r < 8; r++) axpby(1.0, Y0[r], 0.5 * h, k1[r], Y(r));
+      for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], 0.5 * h, k1[r], Y(r));
       after_stage();
       L(k2);
-      for (int r = 0; r < 8; r++) axpby(1.0, Y0[r], 0.5 * h, k2[r], Y(r));
+      for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], 0.5 * h, k2[r], Y(r));
       after_stage();
       L(k3);
-      for (int r = 0; r < 8; r++) axpby(1.0, Y0[r], h, k3[r], Y(r));
+      for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], h, k3[r], Y(r));
       after_stage();
       L(k4);
-      for (int r = 0; r < 8; r++) {
+      for (int r = 0; r < 9; r++) {
         std::vector<double>& y = Y(r);
         for (size_t q = 0; q < NP; q++)
           y[q] = Y0[r][q] +
@@ -1112,6 +1189,7 @@ int ref_create(int nx, int ny, int nz, int ghosts, const double dx[3], const ref
     h->A[d].assign(h->NP, 0.0);
     for (int r = 0; r < 8; r++) h->F[d][r].assign(h->NP, 0.0);
   }
+  h->Psi.assign(h->NP, 0.0);
   for (auto& v : h->U) v.assign(h->NP, 0.0);
   h->mask.assign(h->NP, 0);
   *out = h;
@@ -1165,6 +1243,7 @@ int ref_set_prims(ref_grmhd* h, const double* const field[8]) {
     std::fill(h->A[d].begin(), h->A[d].end(), 0.0);
     std::fill(h->B0[d].begin(), h->B0[d].end(), 0.0);
   }
+  std::fill(h->Psi.begin(), h->Psi.end(), 0.0);
   if (haveB) {
     // G16: static face field B~0 = 2-point mean along the component's own axis of
     // sqrt(gamma_c) B^i_c, on faces 0..n_d, then ghost faces by wrap / copy.
@@ -1268,6 +1347,12 @@ int ref_get_vecpot(ref_grmhd* h, double* const field[3]) {
   return 0;
 }
 
+int ref_get_psi(ref_grmhd* h, double* field) {
+  if (!h || !field) return -1;
+  std::memcpy(field, h->Psi.data(), h->NP * sizeof(double));
+  return 0;
+}
+
 int ref_get_bface(ref_grmhd* h, double* const field[3]) {
   if (!h || !field) return -1;
   for (int d = 0; d < 3; d++) std::memcpy(field[d], h->Bf[d].data(), h->NP * sizeof(double));
@@ -1279,6 +1364,8 @@ int ref_set_option(ref_grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "fixed_dt") == 0) { h->fixed_dt = value; return 0; }
   if (std::strcmp(key, "c2p_backup") == 0) { h->c2p_backup = value != 0.0; return 0; }
   if (std::strcmp(key, "emf") == 0) { h->emf = value != 0.0; return 0; }
+  if (std::strcmp(key, "gauge") == 0) { h->gauge = value != 0.0; return 0; }
+  if (std::strcmp(key, "lorenz_xi") == 0) { h->lorenz_xi = value; return 0; }
   return -1;
 }
 
@@ -1299,6 +1386,16 @@ int ref_rhs(ref_grmhd* h, double* const dU[5], double* const dA[3]) {
   h->rhs(k, k + 5);
   for (int r = 0; r < 5; r++) copy_out_cc(h, k[r], dU[r]);
   for (int d = 0; d < 3; d++) std::memcpy(dA[d], k[5 + d].data(), h->NP * sizeof(double));
+  return 0;
+}
+
+int ref_rhs_gauge(ref_grmhd* h, double* const dA[3], double* dPsi) {
+  if (!h || !dA || !dPsi) return -1;
+  if (!h->have_metric || !h->have_prims) return -3;
+  std::vector<double> k[8], kp;
+  h->rhs(k, k + 5, &kp);
+  for (int d = 0; d < 3; d++) std::memcpy(dA[d], k[5 + d].data(), h->NP * sizeof(double));
+  std::memcpy(dPsi, kp.data(), h->NP * sizeof(double));
   return 0;
 }
 

@@ -43,6 +43,7 @@ int ref_step_until(ref_grmhd* h, double t_end, double cfl, int* nsteps_done);
 int ref_get_prims(ref_grmhd* h, double* const field[8]);
 int ref_get_cons(ref_grmhd* h, double* const field[8]);
 int ref_get_vecpot(ref_grmhd* h, double* const field[3]);
+int ref_get_psi(ref_grmhd* h, double* field); /* Psi_mhd on vertices (staggered shape), option "gauge" = 1 */
 int ref_set_option(ref_grmhd* h, const char* key, double value);
 int ref_get_stats(ref_grmhd* h, ref_stats* out);
 void ref_set_num_threads(int n); /* OpenMP threads for the cell loops (1 = the oracle proper) */
@@ -53,6 +54,9 @@ int ref_get_num_threads(void);
  * interior cells, 0 elsewhere) and 3 staggered arrays (d/dt A_i = -E_i; edges bounding an
  * interior face, 0 elsewhere). */
 int ref_rhs(ref_grmhd* h, double* const dU[5], double* const dA[3]);
+/* d/dt A_i including the gauge term of eq. (31) and d/dt Psi_mhd of eq. (32) (option "gauge");
+ * xi = lorenz_xi / (dt of the last step), 0 before the first step */
+int ref_rhs_gauge(ref_grmhd* h, double* const dA[3], double* dPsi);
 /* stored numerical fluxes of the current state: flux[d][r], d = direction, r = 0..7 rows
  * (D,S_x,S_y,S_z,tau,B^x,B^y,B^z), staggered-shape arrays, densitised F~ = sqrt(gamma_f) F^ */
 int ref_fluxes(ref_grmhd* h, double* const flux[24]);

@@ -172,6 +172,11 @@ class RefSolver:
     def get_vecpot(self):
         return self._get(lib().ref_get_vecpot, 3, self.st_shape)
 
+    def get_psi(self):
+        out = np.zeros(self.st_shape)
+        self._chk(lib().ref_get_psi(self.h, _dp(out)), "ref_get_psi")
+        return out
+
     def get_bface(self):
         return self._get(lib().ref_get_bface, 3, self.st_shape)
 
@@ -188,6 +193,12 @@ class RefSolver:
         dA = [np.zeros(self.st_shape) for _ in range(3)]
         self._chk(lib().ref_rhs(self.h, _ptr_array(dU, 5), _ptr_array(dA, 3)), "ref_rhs")
         return dU, dA
+
+    def rhs_gauge(self):
+        dA = [np.zeros(self.st_shape) for _ in range(3)]
+        dPsi = np.zeros(self.st_shape)
+        self._chk(lib().ref_rhs_gauge(self.h, _ptr_array(dA, 3), _dp(dPsi)), "ref_rhs_gauge")
+        return dA, dPsi
 
     def fluxes(self):
         fl = [np.zeros(self.st_shape) for _ in range(24)]
