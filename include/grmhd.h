@@ -135,8 +135,14 @@ int grmhd_step_until(grmhd* h, double t_end, double cfl, int* nsteps_done);
 int grmhd_get_prims(grmhd* h, double* const field[8]);
 int grmhd_get_cons(grmhd* h, double* const field[8]);
 int grmhd_get_vecpot(grmhd* h, double* const field[3]);
+/* Psi_mhd = sqrt(gamma) Phi of the generalised Lorenz gauge: one staggered-shape
+ * array, vertex (i,j,k) = (i-1/2, j-1/2, k-1/2), incl. filled ghosts; zero in the algebraic gauge. */
+int grmhd_get_psi(grmhd* h, double* field);
 
 /* Keys: "fixed_dt" (> 0: use this dt instead of the CFL reduction; 0 = off);
+ * "gauge" (0 default: algebraic gauge, d_t A_i = -E_i; 1: generalised Lorenz gauge,
+ * eqs (31)-(32) PAPER.md:212-227, Psi_mhd on the vertices as a ninth evolved component; B is
+ * the same in both to round-off), "lorenz_xi" (xi = lorenz_xi / dt, default 1.5);
  * "emf" (0 default: electric field on the edges by flux-CT, R10; 1: upwind constrained
  * transport, eqs (33)-(35) PAPER.md:229-250 -- the flux kernels then also store a_+, a_- and the
  * upwind transverse velocities of every face on a 3-cell transverse apron, and the edges are

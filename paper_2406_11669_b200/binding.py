@@ -21,7 +21,7 @@ _ERRNAME = {EINVAL: "GRMHD_EINVAL", ENOMEM: "GRMHD_ENOMEM", ESTATE: "GRMHD_ESTAT
 
 EXPORTS = ["grmhd_workspace_bytes", "grmhd_create", "grmhd_destroy", "grmhd_set_metric",
            "grmhd_set_prims", "grmhd_set_vecpot", "grmhd_set_mask", "grmhd_step",
-           "grmhd_step_until", "grmhd_get_prims", "grmhd_get_cons", "grmhd_get_vecpot",
+           "grmhd_step_until", "grmhd_get_prims", "grmhd_get_cons", "grmhd_get_vecpot", "grmhd_get_psi",
            "grmhd_set_option", "grmhd_get_stats", "grmhd_get_kernel_times", "grmhd_launch_count", "grmhd_last_error",
            "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_con2prim1d_batch", "grmhd_dfma_peak"]
 
@@ -78,6 +78,7 @@ def lib():
         for nm in ("grmhd_set_metric", "grmhd_set_prims", "grmhd_set_vecpot", "grmhd_get_prims",
                    "grmhd_get_cons", "grmhd_get_vecpot"):
             getattr(L, nm).argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.grmhd_get_psi.argtypes = [C.c_void_p, C.c_void_p]
         L.grmhd_destroy.argtypes = [C.c_void_p]
         L.grmhd_set_mask.argtypes = [C.c_void_p, C.c_void_p]
         L.grmhd_step.argtypes = [C.c_void_p, C.c_int, C.c_double]
@@ -238,6 +239,12 @@ class Solver:
 
     def get_vecpot(self, out=None, host=False):
         return self._get(lib().grmhd_get_vecpot, "grmhd_get_vecpot", 3, self.st_shape, out, host)
+
+    def get_psi(self):
+        """Psi_mhd of the generalised Lorenz gauge on the vertices (staggered shape)."""
+        out = torch.empty(self.st_shape, dtype=torch.float64, device=self.device)
+        self._chk(lib().grmhd_get_psi(self.h, C.c_void_p(out.data_ptr())), "grmhd_get_psi")
+        return out
 
     def stats(self) -> dict:
         s = GrmhdStats()

@@ -69,7 +69,8 @@ __device__ __forceinline__ double uct_bracket(const double* __restrict__ base, c
 // One thread per edge: blockIdx.z = 3 k + comp; E_comp = -[a-bracket] + [b-bracket] with
 // (a, b, comp) cyclic, then R11 d_t A_comp = -E_comp and the RK combination.
 __global__ void __launch_bounds__(256)
-k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk) {
+k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk,
+          int gauge) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   const int k = blockIdx.z / 3;
@@ -80,7 +81,57 @@ k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, Rk
   const int a = (comp + 1) % 3, b = (comp + 2) % 3;
   const long long sa = g.stride(a), sb = g.stride(b);
   const double E = -uct_bracket(base, g, a, b, c, sa, sb) + uct_bracket(base, g, b, a, c, sb, sa);
-  rk_apply(base, g, 5 + comp, c, -E, st->dt, rk);
+  double rhs = -E;
+  if (gauge) {  // eq. (31): - d_comp G_A
+    const double* GA = fld(base, g, F_GV);
+    rhs -= (GA[c + g.stride(comp)] - GA[c]) * g.idx[comp];
+  }
+  rk_apply(base, g, 5 + comp, c, rhs, st->dt, rk);
+}
+
+// ------------------------------------------------------------ generalised Lorenz gauge
+// Row F3; readings G29-G32 of DESIGN.md.  One thread per vertex
+// (i-1/2, j-1/2, k-1/2), i in [-1, nx+1] etc.: the metric as the mean of the 8 cells around the
+// vertex (G29), A_j as the mean of the two edges of its own axis ending there (G30), then
+//   G_A = alpha Psi/sqrt(gamma) - beta^j A_j                    (eq. 31)
+//   F_Psi^d = alpha sqrt(gamma) gamma^{dl} A_l - beta^d Psi     (eq. 32)
+// stored with alpha in the five vertex fields F_GV for k_update / k_emf_uct.
+__global__ void __launch_bounds__(128)
+k_gauge_vertex(double* __restrict__ base, Geom g) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - 1;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y - 1;
+  const int k = blockIdx.z - 1;
+  if (i > g.nx + 1 || j > g.ny + 1) return;
+  const long long c = g.at(i, j, k);
+  const long long sy = g.sy, sz = g.sz;
+  double m[10];
+#pragma unroll
+  for (int f = 0; f < 10; f++) {
+    const double* q = fld(base, g, F_MET + f) + c;
+    double acc = 0.0;
+#pragma unroll
+    for (int b = 0; b < 8; b++) acc += q[-(b & 1) - ((b >> 1) & 1) * sy - ((b >> 2) & 1) * sz];
+    m[f] = 0.125 * acc;
+  }
+  Met M;
+  M.a = m[0]; M.bx = m[1]; M.by = m[2]; M.bz = m[3];
+  M.gxx = m[4]; M.gxy = m[5]; M.gxz = m[6]; M.gyy = m[7]; M.gyz = m[8]; M.gzz = m[9];
+  const double det = det_gamma(M);
+  const double sg = sqrt(det);
+  const Sym3 gu = inv_gamma(M, 1.0 / det);
+  const double* Ax = fld(base, g, F_Y + 5);
+  const double* Ay = fld(base, g, F_Y + 6);
+  const double* Az = fld(base, g, F_Y + 7);
+  const double ax = 0.5 * (Ax[c - 1] + Ax[c]);
+  const double ay = 0.5 * (Ay[c - sy] + Ay[c]);
+  const double az = 0.5 * (Az[c - sz] + Az[c]);
+  const double psi = fld(base, g, F_Y + 8)[c];
+  fld(base, g, F_GV + 0)[c] = M.a * psi / sg - (M.bx * ax + M.by * ay + M.bz * az);
+  const double asg = M.a * sg;
+  fld(base, g, F_GV + 1)[c] = asg * (gu.xx * ax + gu.xy * ay + gu.xz * az) - M.bx * psi;
+  fld(base, g, F_GV + 2)[c] = asg * (gu.xy * ax + gu.yy * ay + gu.yz * az) - M.by * psi;
+  fld(base, g, F_GV + 3)[c] = asg * (gu.xz * ax + gu.yz * ay + gu.zz * az) - M.bz * psi;
+  fld(base, g, F_GV + 4)[c] = M.a;
 }
 
 }  // namespace gk

@@ -145,6 +145,8 @@ Eos make_eos(const grmhd_opts& o) {
   E.riemann = o.riemann;
   E.c2p_backup = 0;
   E.emf = 0;
+  E.gauge = 0;
+  E.lorenz_xi = 1.5;
   return E;
 }
 
@@ -249,11 +251,15 @@ FillArgs fill_prims() {
   for (int r = 0; r < 5; r++) { fa.id[r] = F_P + r; fa.stag[r] = 0; fa.kind[r] = 0; }
   return fa;
 }
-FillArgs fill_vecpot() {
+FillArgs fill_vecpot(bool with_psi = false) {
   FillArgs fa{};
   fa.nf = 3;
   const int st[3] = {2 | 4, 1 | 4, 1 | 2};  // A_x on (y,z)-staggered edges, ...
   for (int d = 0; d < 3; d++) { fa.id[d] = F_Y + 5 + d; fa.stag[d] = st[d]; fa.kind[d] = 1; }
+  if (with_psi) {  // Psi_mhd on the vertices: wrap / copy (G29)
+    fa.id[3] = F_Y + 8; fa.stag[3] = 1 | 2 | 4; fa.kind[3] = 0;
+    fa.nf = 4;
+  }
   return fa;
 }
 
@@ -271,7 +277,7 @@ int after_stage(grmhd* h, bool want_speed) {
   const Geom& g = h->g;
   int rc;
   KT(KG_BFIELD, {
-    rc = fill_ghosts(h, fill_vecpot());
+    rc = fill_ghosts(h, fill_vecpot(h->E.gauge != 0));
     if (rc) return rc;
   });
   KT(KG_C2P, {
@@ -491,13 +497,20 @@ int one_step(grmhd* h) {
     int rc = compute_fluxes(h);
     if (rc) return rc;
     KT(KG_UPDATE, {
-      const int nrows = h->E.emf ? 5 : 8;  // with the upwind CT the edges have their own kernel
+      const int gauge = h->E.gauge;
+      if (gauge) {  // G_A, F_Psi^j and alpha on the vertices -1 .. n+1
+        k_gauge_vertex<<<grd3(g.nx + 3, g.ny + 3, g.nz + 3), blk3(), 0, h->s>>>(h->base, g);
+        CKL("k_gauge_vertex");
+      }
+      // with the upwind CT the edges have their own kernel; the Lorenz gauge adds the Psi row
+      const int nrows = (h->E.emf ? 5 : 8) + (gauge ? 1 : 0);
       k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, nrows * (g.nz + 1)),
-                 dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], nrows);
+                 dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], nrows, gauge,
+                                             h->E.lorenz_xi);
       CKL("k_update");
       if (h->E.emf) {
         k_emf_uct<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 3 * (g.nz + 1)),
-                    dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s]);
+                    dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], gauge);
         CKL("k_emf_uct");
       }
     });
@@ -615,6 +628,7 @@ int grmhd_set_prims(grmhd* h, const double* const field[8]) {
   if ((rc = fill_ghosts(h, fill_prims()))) return rc;
   for (int d = 0; d < 3; d++) {
     if ((rc = zero_field(h, F_Y + 5 + d))) return rc;
+    if (d == 0 && (rc = zero_field(h, F_Y + 8))) return rc;  // Psi_mhd = 0
     if ((rc = zero_field(h, F_B0 + d))) return rc;
   }
   if (haveB) {
@@ -745,6 +759,16 @@ int grmhd_get_vecpot(grmhd* h, double* const field[3]) {
   return GRMHD_OK;
 }
 
+int grmhd_get_psi(grmhd* h, double* field) {
+  if (!h) return GRMHD_EINVAL;
+  if (!field) return fail(h, GRMHD_EINVAL, "get_psi: NULL field");
+  if (h->dirty) { int rc0 = init_state(h); if (rc0) return rc0; }
+  int rc = copy_out(h, F_Y + 8, field, true, 0);
+  if (rc) return rc;
+  CK(cudaStreamSynchronize(h->s));
+  return GRMHD_OK;
+}
+
 int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (!h || !key) return GRMHD_EINVAL;
   if (std::strcmp(key, "fixed_dt") == 0) {
@@ -754,6 +778,16 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "flux_kernel") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
     h->flux_impl = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "gauge") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: gauge is 0 or 1");
+    h->E.gauge = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "lorenz_xi") == 0) {
+    if (!(value >= 0.0)) return fail(h, GRMHD_EINVAL, "set_option: lorenz_xi < 0");
+    h->E.lorenz_xi = value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "emf") == 0) {

@@ -109,16 +109,32 @@ __device__ __forceinline__ void rk_apply(double* __restrict__ base, const Geom& 
 // (kernels_aux.cuh) when the primitives they depend on were recovered.
 __global__ void __launch_bounds__(256)
 k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk,
-         int nrows) {
+         int nrows, int gauge, double lorenz_xi) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z / nrows;  // nrows = 8, or 5 when k_emf_uct updates the edges
+  // nrows = 8 (5 hydro rows + 3 edges), 5 when k_emf_uct updates the edges; in the Lorenz gauge
+  // one more row, the last: Psi_mhd on the vertices
+  const int k = blockIdx.z / nrows;
   const int r = blockIdx.z % nrows;
   if (i > g.nx || j > g.ny) return;
   const long long c = g.at(i, j, k);
   const double h = st->dt;
   const long long sy = g.sy, sz = g.sz;
   double rhs;
+  if (gauge && r == nrows - 1) {
+    // eq. (32): d_t Psi = -d_j F_Psi^j - xi alpha Psi at the vertex (G32), xi = lorenz_xi / dt
+    const double* Fx = fld(base, g, F_GV + 1);
+    const double* Fy = fld(base, g, F_GV + 2);
+    const double* Fz = fld(base, g, F_GV + 3);
+    double div = (Fx[c + 1] - Fx[c - 1]) * (0.5 * g.idx[0]);
+    div += (Fy[c + sy] - Fy[c - sy]) * (0.5 * g.idx[1]);
+    div += (Fz[c + sz] - Fz[c - sz]) * (0.5 * g.idx[2]);
+    const double xi = h > 0.0 ? lorenz_xi / h : 0.0;
+    rhs = -div - xi * fld(base, g, F_GV + 4)[c] * fld(base, g, F_Y + 8)[c];
+    rk_apply(base, g, 8, c, rhs, h, rk);
+    return;
+  }
+  const double* GA = fld(base, g, F_GV);  // eq. (31): d_t A_i = -E_i - d_i G_A (G31)
   if (r < 5) {
     if (i >= g.nx || j >= g.ny || k >= g.nz) return;
     // R8: L(U~) = -sum_d (F~_{i+1/2} - F~_{i-1/2})/dx_d + alpha sqrt(gamma) S, eq. (17)
@@ -138,16 +154,19 @@ k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkS
     const double* FyBz = fld(base, g, F_FY + 5);
     const double* FzBy = fld(base, g, F_FZ + 6);
     rhs = -0.25 * (-FyBz[c - sz] - FyBz[c] + FzBy[c - sy] + FzBy[c]);
+    if (gauge) rhs -= (GA[c + 1] - GA[c]) * g.idx[0];
   } else if (r == 6) {
     if (j >= g.ny) return;  // E_y at (i-1/2, j, k-1/2)
     const double* FzBx = fld(base, g, F_FZ + 5);
     const double* FxBz = fld(base, g, F_FX + 6);
     rhs = -0.25 * (-FzBx[c - 1] - FzBx[c] + FxBz[c - sz] + FxBz[c]);
+    if (gauge) rhs -= (GA[c + sy] - GA[c]) * g.idx[1];
   } else {
     if (k >= g.nz) return;  // E_z at (i-1/2, j-1/2, k)
     const double* FxBy = fld(base, g, F_FX + 5);
     const double* FyBx = fld(base, g, F_FY + 6);
     rhs = -0.25 * (-FxBy[c - sy] - FxBy[c] + FyBx[c - 1] + FyBx[c]);
+    if (gauge) rhs -= (GA[c + sz] - GA[c]) * g.idx[2];
   }
   rk_apply(base, g, r, c, rhs, h, rk);
 }

@@ -40,17 +40,18 @@ enum FieldId {
   F_BC = 21,    // 3 : Eulerian B^i at cell centres
   F_BF = 24,    // 3 : densitised B~^d on d-faces (total)
   F_B0 = 27,    // 3 : static part B~0 (G16)
-  F_Y = 30,     // 8 : evolved D~, S~_j, tau~ (cells) and A_i (edges)
-  F_Y0 = 38,    // 8 : RK register Y^0
-  F_FX = 46,    // 7 : stored x-fluxes: D,S_x,S_y,S_z,tau rows + B^y, B^z rows
-  F_FY = 53,    // 7 : y-fluxes (+ B^z, B^x rows)
-  F_FZ = 60,    // 7 : z-fluxes (+ B^x, B^y rows)
-  F_SRC = 67,   // 4 : alpha sqrt(gamma) S of eq. (19) for the rows S_x, S_y, S_z, tau (cells)
-  F_W = 71,     // 12: upwind-CT face data, 4 per direction d: a_+, a_- (eq. 34) and the upwind
+  F_Y = 30,     // 9 : evolved D~, S~_j, tau~ (cells), A_i (edges), Psi_mhd (vertices, Lorenz gauge)
+  F_Y0 = 39,    // 9 : RK register Y^0
+  F_FX = 48,    // 7 : stored x-fluxes: D,S_x,S_y,S_z,tau rows + B^y, B^z rows
+  F_FY = 55,    // 7 : y-fluxes (+ B^z, B^x rows)
+  F_FZ = 62,    // 7 : z-fluxes (+ B^x, B^y rows)
+  F_SRC = 69,   // 4 : alpha sqrt(gamma) S of eq. (19) for the rows S_x, S_y, S_z, tau (cells)
+  F_W = 73,     // 12: upwind-CT face data, 4 per direction d: a_+, a_- (eq. 34) and the upwind
                 //     transverse velocities vbar^{(d+1)%3}, vbar^{(d+2)%3} (eq. 33); F_W + 4 d + r
-  F_KS = 83,    // 8 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
-  F_END_RK23 = 83,
-  F_END_RK4 = 91
+  F_GV = 85,    // 5 : Lorenz gauge, on vertices: G_A (eq. 31), F_Psi^x,y,z (eq. 32), alpha
+  F_KS = 90,    // 9 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
+  F_END_RK23 = 90,
+  F_END_RK4 = 99
 };
 
 // device-resident scalars of a handle

@@ -36,6 +36,8 @@ struct Eos {
   int recon;        // 0 minmod, 1 PPM
   int flatten;
   int riemann;      // 0 HLLE eq. (29), 1 LxF eq. (30)
+  int gauge;        // 0 algebraic gauge, 1 generalised Lorenz gauge (eqs 31-32)
+  double lorenz_xi; // xi = lorenz_xi / dt
   int emf;          // 0 flux-CT (R10), 1 upwind CT (eqs 33-35)
   int c2p_backup;   // 1: 1-D scheme when the 2-D Newton iteration fails
 };
