@@ -40,6 +40,11 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample-n", type=int, default=48)
+    ap.add_argument("--set", action="append", default=[], metavar="KEY=VALUE",
+                    help="grmhd_set_option before the run, e.g. --set emf=1 (upwind CT), "
+                         "--set gauge=1 (Lorenz gauge), --set c2p_backup=1")
+    ap.add_argument("--no-point-kernels", action="store_true",
+                    help="skip the FP64 peak and config-4b con2prim measurements")
     return ap.parse_args()
 
 
@@ -214,6 +219,29 @@ def whole_job_value(ncells, stages, steps, world, ms):
     return world * ncells * stages * steps / (ms * 1e-3)
 
 
+def point_kernels(binding, torch, n=1 << 22):
+    """FP64 pipe peak (dependent-free DFMA loop) and 'config 4b': the two con2prim
+    schemes alone on n iid states with the config-4 marginals, device resident."""
+    from paper_2406_11669_b200 import workloads as wl
+    out = {"fp64_peak_tflops_measured": binding.dfma_peak()}
+    prim, met = wl.c2p_states(n)
+    o = binding.make_opts(gamma_ad=5.0 / 3.0, rho_atm=1e-10, p_floor=1e-10, w_max=100.0)
+    P, M = torch.from_numpy(prim).cuda(), torch.from_numpy(met).cuda()
+    U = binding.prim2con_batch(P, M, o)
+    for name, fn in (("con2prim_2d", binding.con2prim_batch), ("con2prim_1d", binding.con2prim1d_batch)):
+        fn(U, M, o)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            _, st, it = fn(U, M, o)
+        e1.record()
+        e1.synchronize()
+        ms = e0.elapsed_time(e1) / 5
+        out[name] = {"states": n, "ms": ms, "states_per_s": n / (ms * 1e-3),
+                     "mean_iterations": float(it.double().mean()), "failed": int((st & 2).ne(0).sum())}
+    return out
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -236,6 +264,11 @@ def run_b200(args):
     s.set_metric(w.metric)
     if w.mask is not None:
         s.set_mask(w.mask)
+    options = {}
+    for kv in args.set:
+        key, val = kv.split("=", 1)
+        s.set_option(key, float(val))
+        options[key] = float(val)
 
     def reset():
         s.set_prims(h_prims)
@@ -295,6 +328,9 @@ def run_b200(args):
            "ms_per_step": ms_e2e / k_e2e,
            "call": "set_prims[+set_vecpot](pinned host) -> step(1) -> get_cons(pinned host)"}
     s.close()
+    point = None
+    if rank == 0 and not args.no_point_kernels:
+        point = point_kernels(binding, torch)
     if world > 1:
         dist.destroy_process_group()
     if rank != 0:
@@ -335,7 +371,8 @@ def run_b200(args):
                        "l2": "inputs larger than L2 (every kernel streams > 126 MB)"
                              if w.ncells >= 128 ** 3 else "working set fits L2 (latency-bound config)",
                        "us_per_substep": 1e3 * ms / (args.steps * w.stages)},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "options": options,
+            "point_kernels": point,
             "roofline": roofline, "kernels": kernels,
             "stats": {k: st[k] for k in ("t", "dt", "c2p_fail", "p_fix", "atmo", "w_cap",
                                          "c2p_maxiter")}}
