@@ -71,7 +71,8 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
 //           blocks and option combinations only).
 //   mode 1: only the 2 ap apron columns t0 < 0 and t0 >= n_t0 that the 32-wide groups of
 //           k_flux_tma leave out.
-template <int D, int RECON>
+// UCT (compile time, as in k_flux_tma): also store the upwind-CT face rows of F_W.
+template <int D, int RECON, bool UCT>
 __global__ void __launch_bounds__(FX_THREADS, FX_MINB)
 k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems, int ap,
             int mode) {
@@ -149,18 +150,18 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
   // slots 5, 6 hold B^{(D+1)%3}, B^{(D+2)%3}
   ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
              D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]), M,
-             gdd, E, UL, GL, lmL, lpL, vtL);
+             gdd, E, UL, GL, lmL, lpL, UCT ? vtL : nullptr);
   ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
              D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]), M,
-             gdd, E, UR, GR, lmR, lpR, vtR);
+             gdd, E, UR, GR, lmR, lpR, UCT ? vtR : nullptr);
   double out[7];
-  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out, apm);
+  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out, UCT ? apm : nullptr);
   if (lane >= 3 && lane < 3 + FX_VALID && c <= nD) {
     double* o = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
     for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
-    if (E.emf) ft_store_uct(fld(base, g, F_W + 4 * D) + idx, NPA, apm, vtL, vtR);
+    if (UCT) ft_store_uct(fld(base, g, F_W + 4 * D) + idx, NPA, apm, vtL, vtR);
   }
   }  // items
 }

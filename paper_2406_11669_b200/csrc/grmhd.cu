@@ -352,8 +352,12 @@ int launch_flux_xrow(grmhd* h, int mode) {
   const long long npen = (long long)(mode ? 2 * ap : nt0 + 2 * ap) * (nt1 + 2 * ap);
   const long long nitems = npen * nsd;
   const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
-  k_flux_xrow<D, RECON><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd, nitems,
-                                                                ap, mode);
+  if (h->E.emf)
+    k_flux_xrow<D, RECON, true><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd,
+                                                                        nitems, ap, mode);
+  else
+    k_flux_xrow<D, RECON, false><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd,
+                                                                         nitems, ap, mode);
   h->launches++;
   return GRMHD_OK;
 }
@@ -504,9 +508,15 @@ int one_step(grmhd* h) {
       }
       // with the upwind CT the edges have their own kernel; the Lorenz gauge adds the Psi row
       const int nrows = (h->E.emf ? 5 : 8) + (gauge ? 1 : 0);
-      k_update<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, nrows * (g.nz + 1)),
-                 dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], nrows, gauge,
-                                             h->E.lorenz_xi);
+      const dim3 ug((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, nrows * (g.nz + 1)), ub(128, 2, 1);
+      if (nrows == 8)
+        k_update<8, false><<<ug, ub, 0, h->s>>>(h->base, g, h->dst, st[s], h->E.lorenz_xi);
+      else if (nrows == 5)
+        k_update<5, false><<<ug, ub, 0, h->s>>>(h->base, g, h->dst, st[s], h->E.lorenz_xi);
+      else if (nrows == 9)
+        k_update<9, true><<<ug, ub, 0, h->s>>>(h->base, g, h->dst, st[s], h->E.lorenz_xi);
+      else
+        k_update<6, true><<<ug, ub, 0, h->s>>>(h->base, g, h->dst, st[s], h->E.lorenz_xi);
       CKL("k_update");
       if (h->E.emf) {
         k_emf_uct<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 3 * (g.nz + 1)),

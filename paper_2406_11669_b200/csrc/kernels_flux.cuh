@@ -107,9 +107,12 @@ __device__ __forceinline__ void rk_apply(double* __restrict__ base, const Geom& 
 // coalesced along x, the row is uniform per block (no divergence) and the register need is
 // small enough for full occupancy.  The sources alpha sqrt(gamma) S were stored by k_post
 // (kernels_aux.cuh) when the primitives they depend on were recovered.
+template <int NROWS, bool GAUGE>
 __global__ void __launch_bounds__(256)
 k_update(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk,
-         int nrows, int gauge, double lorenz_xi) {
+         double lorenz_xi) {
+  constexpr int nrows = NROWS;
+  constexpr bool gauge = GAUGE;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y * blockDim.y + threadIdx.y;
   // nrows = 8 (5 hydro rows + 3 edges), 5 when k_emf_uct updates the edges; in the Lorenz gauge
