@@ -14,16 +14,18 @@ namespace gk {
 // the two a-faces that share the edge.  c = index of the edge, sa / sb = strides of a and b.
 // G8 without flattening on the 6 values s[0..5] around a position: L = q^+ of cell 2, R = q^- of
 // cell 3; branch free, same arithmetic as FtMarch::step.
-__device__ __forceinline__ void uct_limit(double q, double& qm, double& qp) {
+// monotonised q^+ (UPPER = true) or q^- of a cell from its two interface values
+template <bool UPPER>
+__device__ __forceinline__ double uct_limit(double q, double qm, double qp) {
   const double a = qp - q, b = q - qm;
-  const double aa = fabs(a), ab = fabs(b);
   const bool flat = ft_opposite(a, b);
-  const bool fixm = ab > 2.0 * aa;
-  const bool fixp = aa > 2.0 * ab;
-  const double qm2 = fma(-2.0, a, q);
-  const double qp2 = fma(2.0, b, q);
-  qm = ft_sel(flat, q, ft_sel(fixm, qm2, qm));
-  qp = ft_sel(flat, q, ft_sel(fixp, qp2, qp));
+  if (UPPER) {
+    const bool fixp = fabs(a) > 2.0 * fabs(b);
+    return ft_sel(flat, q, ft_sel(fixp, fma(2.0, b, q), qp));
+  } else {
+    const bool fixm = fabs(b) > 2.0 * fabs(a);
+    return ft_sel(flat, q, ft_sel(fixm, fma(-2.0, a, q), qm));
+  }
 }
 __device__ __forceinline__ void uct_recon6(const double s[6], double& L, double& R) {
   const double d0 = s[1] - s[0], d1 = s[2] - s[1], d2 = s[3] - s[2], d3 = s[4] - s[3],
@@ -33,12 +35,8 @@ __device__ __forceinline__ void uct_recon6(const double s[6], double& L, double&
   const double i12 = 0.5 * (s[1] + s[2]) - (m2 - m1) * (1.0 / 6.0);
   const double i23 = 0.5 * (s[2] + s[3]) - (m3 - m2) * (1.0 / 6.0);
   const double i34 = 0.5 * (s[3] + s[4]) - (m4 - m3) * (1.0 / 6.0);
-  double qm = i12, qp = i23;
-  uct_limit(s[2], qm, qp);
-  L = qp;
-  qm = i23; qp = i34;
-  uct_limit(s[3], qm, qp);
-  R = qm;
+  L = uct_limit<true>(s[2], i12, i23);   // q^+ of the lower cell
+  R = uct_limit<false>(s[3], i23, i34);  // q^- of the upper cell
 }
 
 __device__ __forceinline__ double uct_bracket(const double* __restrict__ base, const Geom& g,
