@@ -2,6 +2,7 @@
 // (eqs 33-35; readings G26-G28 of DESIGN.md) and the update of A_i.
 #pragma once
 #include "flux_tma.cuh"
+#include "flux_xrow.cuh"
 #include "kernels_flux.cuh"
 
 namespace gk {
@@ -80,6 +81,181 @@ k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, Rk
   const long long sa = g.stride(a), sb = g.stride(b);
   const double E = -uct_bracket(base, g, a, b, c, sa, sb) + uct_bracket(base, g, b, a, c, sb, sa);
   double rhs = -E;
+  if (gauge) {  // eq. (31): - d_comp G_A
+    const double* GA = fld(base, g, F_GV);
+    rhs -= (GA[c + g.stride(comp)] - GA[c]) * g.idx[comp];
+  }
+  rk_apply(base, g, 5 + comp, c, rhs, st->dt, rk);
+}
+
+// ---- the same electric field, every face -> edge parabola built once --------------------
+// k_emf_uct above rebuilds each parabola in both edges that use it (and each slope four
+// times).  The passes below take one reconstruction axis A at a time and compute the two
+// brackets of eq. (35) that reconstruct along A, for every edge index (i,j,k) in [0, n]:
+//   br(A, A+1) -> -E_{A+2},   br(A, A+2) -> +E_{A+1}
+// into three scratch fields (the flux-CT B rows F_FX+5, F_FY+5, F_FZ+5, unused with the upwind
+// CT, hold E_x, E_y, E_z).  Pass order x, y, z; `wr` bit 0 / bit 1 = the first / second
+// bracket writes (first contribution) instead of adding.  k_emf_apply then does R11 + RK.
+__device__ __forceinline__ double* uct_escratch(double* base, const Geom& g, int comp) {
+  return fld(base, g, comp == 0 ? F_FX + 5 : (comp == 1 ? F_FY + 5 : F_FZ + 5));
+}
+__device__ __forceinline__ double uct_combine(double ap, double am, double vL, double vR,
+                                              double BL, double BR) {
+  const double cs = ap + am;
+  const bool deg = cs < 1e-300;
+  const double w = ft_rcp(deg ? 1.0 : cs);
+  const double full = (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) * w;
+  return deg ? 0.5 * (vL * BL + vR * BR) : full;
+}
+__device__ __forceinline__ int uct_vbar_field(int a, int b) {  // vbar^a on the b-faces
+  return F_W + 4 * b + (a == (b + 1) % 3 ? 2 : 3);
+}
+
+// A = 1, 2: lanes along x, one thread per (i, t) column marching along A with the PPM state of
+// the four quantities carried in registers (FtMarch, as in the flux kernels).
+#ifndef UM_MINB
+#define UM_MINB 4
+#endif
+template <int A>
+__global__ void __launch_bounds__(128, UM_MINB)
+k_uct_march(double* __restrict__ base, Geom g, int seglen, int wr, int fin,
+            const DevState* __restrict__ st, RkStage rk, int gauge) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int t = blockIdx.y;
+  if (i > g.nx) return;
+  const int nA = g.n(A);
+  const int m0 = (int)blockIdx.z * seglen, m1 = min(m0 + seglen, nA + 1);
+  constexpr int b1 = (A + 1) % 3, b2 = (A + 2) % 3;
+  constexpr int c1 = (A + 2) % 3, c2 = (A + 1) % 3;  // br1 -> -E_c1, br2 -> +E_c2
+  const long long sA = g.stride(A), s1 = g.stride(b1), s2 = g.stride(b2);
+  const long long c0 = A == 1 ? g.at(i, 0, t) : g.at(i, t, 0);  // position 0 along A
+  const double* q[4] = {fld(base, g, uct_vbar_field(A, b1)) + c0, fld(base, g, F_BF + b1) + c0,
+                        fld(base, g, uct_vbar_field(A, b2)) + c0, fld(base, g, F_BF + b2) + c0};
+  const double* Ap = fld(base, g, F_W + 4 * A) + c0;
+  const double* Am = fld(base, g, F_W + 4 * A + 1) + c0;
+  double* E1 = uct_escratch(base, g, c1) + c0;
+  double* E2 = uct_escratch(base, g, c2) + c0;
+  // which of the two finished components exist at this (i, t): E_x for i < nx, else the index
+  // along the component's own axis (t is the index along b2 for A = 1, along b1 for A = 2)
+  const int tb = A == 1 ? 2 : 1;  // axis of t
+  const bool ok1 = c1 == 0 ? i < g.nx : (c1 == tb ? t < g.n(c1) : true);
+  const bool ok2 = c2 == 0 ? i < g.nx : (c2 == tb ? t < g.n(c2) : true);
+  const double h = st->dt;
+  const double* GA = fld(base, g, F_GV) + c0;
+  FtMarch<1> mv[4];
+#pragma unroll
+  for (int v = 0; v < 4; v++) {
+    mv[v].init(q[v][(m0 - 3) * sA], q[v][(m0 - 2) * sA], q[v][(m0 - 1) * sA], q[v][m0 * sA]);
+    double qm, qp;
+    mv[v].step(q[v][(m0 + 1) * sA], 0.0, false, qm, qp);  // position m0 - 1
+    mv[v].qpp = qp;
+  }
+  // values of the next step, loaded one step ahead
+  double nq[4], na[6];
+  auto fetch = [&](int m) {
+    const long long c = m * sA;
+#pragma unroll
+    for (int v = 0; v < 4; v++) nq[v] = q[v][c + 2 * sA];
+    na[0] = Ap[c]; na[1] = Ap[c - s1]; na[2] = Ap[c - s2];
+    na[3] = Am[c]; na[4] = Am[c - s1]; na[5] = Am[c - s2];
+  };
+  fetch(m0);
+  for (int m = m0; m < m1; m++) {
+    double cq[4], ca[6];
+#pragma unroll
+    for (int v = 0; v < 4; v++) cq[v] = nq[v];
+#pragma unroll
+    for (int v = 0; v < 6; v++) ca[v] = na[v];
+    if (m + 1 < m1) fetch(m + 1);
+    double L[4], R[4];
+#pragma unroll
+    for (int v = 0; v < 4; v++) {
+      double qm, qp;
+      mv[v].step(cq[v], 0.0, false, qm, qp);
+      L[v] = mv[v].qpp;  // q^+ of position m - 1
+      R[v] = qm;         // q^- of position m
+      mv[v].qpp = qp;
+    }
+    const long long c = m * sA;
+    const double br1 = uct_combine(ft_max(ca[0], ca[1]), ft_max(ca[3], ca[4]), L[0], R[0], L[1],
+                                   R[1]);
+    const double br2 = uct_combine(ft_max(ca[0], ca[2]), ft_max(ca[3], ca[5]), L[2], R[2], L[3],
+                                   R[3]);
+    const double e1 = (wr & 1) ? -br1 : E1[c] - br1;
+    const double e2 = (wr & 2) ? br2 : E2[c] + br2;
+    // a component whose second bracket this is goes straight into R11 + RK (no second trip)
+    const bool in1 = ok1 && (c1 != A || m < nA), in2 = ok2 && (c2 != A || m < nA);
+    if (fin & 1) {
+      if (in1) {
+        double rhs = -e1;
+        if (gauge) rhs -= (GA[c + g.stride(c1)] - GA[c]) * g.idx[c1];
+        rk_apply(base, g, 5 + c1, c0 + c, rhs, h, rk);
+      }
+    } else {
+      E1[c] = e1;
+    }
+    if (fin & 2) {
+      if (in2) {
+        double rhs = -e2;
+        if (gauge) rhs -= (GA[c + g.stride(c2)] - GA[c]) * g.idx[c2];
+        rk_apply(base, g, 5 + c2, c0 + c, rhs, h, rk);
+      }
+    } else {
+      E2[c] = e2;
+    }
+  }
+}
+
+// A = 0: lanes along x, the recurrences across lanes by shuffles (fx_recon, as k_flux_xrow):
+// one warp per 27 edge positions of a row (j, k) in [0, ny] x [0, nz].
+__global__ void __launch_bounds__(128)
+k_uct_xrow(double* __restrict__ base, Geom g, int nsd, long long nitems, int wr) {
+  const int lane = threadIdx.x & 31;
+  const long long item = (long long)blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (item >= nitems) return;  // warp uniform
+  const int seg = (int)(item % nsd);
+  const int row = (int)(item / nsd);
+  const int j = row % (g.ny + 1), k = row / (g.ny + 1);
+  const int p = seg * FX_VALID - 3 + lane;
+  const long long c = g.at(min(p, g.nx + G - 1), j, k);
+  constexpr int b1 = 1, b2 = 2;
+  const double qv[4] = {fld(base, g, uct_vbar_field(0, b1))[c], fld(base, g, F_BF + b1)[c],
+                        fld(base, g, uct_vbar_field(0, b2))[c], fld(base, g, F_BF + b2)[c]};
+  double L[4], R[4];
+#pragma unroll
+  for (int v = 0; v < 4; v++) {
+    double qm, qp;
+    fx_recon<1>(qv[v], fx_up(qv[v], 1), fx_dn(qv[v], 1), 0.0, false, qm, qp);
+    L[v] = fx_up(qp, 1);
+    R[v] = qm;
+  }
+  if (lane >= 3 && lane < 3 + FX_VALID && p <= g.nx) {
+    const double* Ap = fld(base, g, F_W + 0);
+    const double* Am = fld(base, g, F_W + 1);
+    const long long s1 = g.sy, s2 = g.sz;
+    const double br1 = uct_combine(ft_max(Ap[c], Ap[c - s1]), ft_max(Am[c], Am[c - s1]), L[0],
+                                   R[0], L[1], R[1]);
+    const double br2 = uct_combine(ft_max(Ap[c], Ap[c - s2]), ft_max(Am[c], Am[c - s2]), L[2],
+                                   R[2], L[3], R[3]);
+    double* E1 = uct_escratch(base, g, 2);
+    double* E2 = uct_escratch(base, g, 1);
+    E1[c] = (wr & 1) ? -br1 : E1[c] - br1;
+    E2[c] = (wr & 2) ? br2 : E2[c] + br2;
+  }
+}
+
+// R11 + RK on the edges from the scratch E (one thread per edge: blockIdx.z = 3 k + comp)
+__global__ void __launch_bounds__(256)
+k_emf_apply(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk,
+            int gauge) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y;
+  const int k = blockIdx.z / 3;
+  const int comp = blockIdx.z % 3;
+  if (i > g.nx || j > g.ny) return;
+  if ((comp == 0 && i >= g.nx) || (comp == 1 && j >= g.ny) || (comp == 2 && k >= g.nz)) return;
+  const long long c = g.at(i, j, k);
+  double rhs = -uct_escratch(base, g, comp)[c];
   if (gauge) {  // eq. (31): - d_comp G_A
     const double* GA = fld(base, g, F_GV);
     rhs -= (GA[c + g.stride(comp)] - GA[c]) * g.idx[comp];

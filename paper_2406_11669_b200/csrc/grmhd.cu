@@ -40,6 +40,8 @@ struct grmhd {
   int ft_conc[18] = {0};  // ... of the TMA-fed instantiations
   CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][.] of the ring stages, per direction
   bool tma_ok = false;
+  int uct_nseg = 16;     // segments of the marching passes along y and z
+  int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
   int xrow = 1;          // x fluxes: 1 k_flux_xrow (lanes along x), 0 as y and z
   int flux_impl = 1;     // 1: k_flux_tma (+ k_flux_march on the apron columns), 0: k_flux_march
   char err[256] = {0};
@@ -518,7 +520,22 @@ int one_step(grmhd* h) {
       else
         k_update<6, true><<<ug, ub, 0, h->s>>>(h->base, g, h->dst, st[s], h->E.lorenz_xi);
       CKL("k_update");
-      if (h->E.emf) {
+      if (h->E.emf && h->uct_passes) {
+        // every face -> edge parabola once: passes along x, y, z, then R11 + RK
+        const int nsd = (g.nx + 1 + FX_VALID - 1) / FX_VALID;
+        const long long nitems = (long long)nsd * (g.ny + 1) * (g.nz + 1);
+        k_uct_xrow<<<(unsigned)((nitems + 3) / 4), 128, 0, h->s>>>(h->base, g, nsd, nitems, 3);
+        CKL("k_uct_xrow");
+        const int nsg = h->uct_nseg;
+        const int sly = (g.ny + 1 + nsg - 1) / nsg, slz = (g.nz + 1 + nsg - 1) / nsg;
+        // pass y finishes E_z, pass z finishes E_y and E_x: those go straight into R11 + RK
+        k_uct_march<1><<<dim3((g.nx + 1 + 127) / 128, g.nz + 1, (g.ny + sly) / sly), 128, 0,
+                         h->s>>>(h->base, g, sly, 1, 2, h->dst, st[s], gauge);
+        CKL("k_uct_march");
+        k_uct_march<2><<<dim3((g.nx + 1 + 127) / 128, g.ny + 1, (g.nz + slz) / slz), 128, 0,
+                         h->s>>>(h->base, g, slz, 0, 3, h->dst, st[s], gauge);
+        CKL("k_uct_march");
+      } else if (h->E.emf) {
         k_emf_uct<<<dim3((g.nx + 1 + 127) / 128, (g.ny + 1 + 1) / 2, 3 * (g.nz + 1)),
                     dim3(128, 2, 1), 0, h->s>>>(h->base, g, h->dst, st[s], gauge);
         CKL("k_emf_uct");
@@ -808,6 +825,15 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "c2p_backup") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: c2p_backup is 0 or 1");
     h->E.c2p_backup = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "uct_nseg") == 0) {
+    if (!(value >= 1.0 && value <= 64.0)) return fail(h, GRMHD_EINVAL, "set_option: uct_nseg");
+    h->uct_nseg = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "uct_passes") == 0) {
+    h->uct_passes = value != 0.0;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "flux_x_rows") == 0) {
