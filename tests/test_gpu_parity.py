@@ -171,6 +171,7 @@ def test_upwind_ct_matches_oracle():
     direction), minmod, RK4, and the x fluxes through the TMA kernel."""
     cases = [(wl.kerr_blob(40), None), (wl.blast(44), None), (wl.c2p_stress(36), None),
              (wl.bns_like(32), None), (wl.kerr_blob(40), {"flux_x_rows": 0.0}),
+             (wl.kerr_blob(40), {"uct_passes": 0.0}),   # the per-edge kernel k_emf_uct
              (wl.alfven_wave(16, 1, 1, axis=0), None), (wl.balsara1(64, 4, 4), None),
              (wl.make(1), None)]          # 128^3: several groups, segments and waves
     for w, extra in cases:
