@@ -147,6 +147,8 @@ int grmhd_get_psi(grmhd* h, double* field);
  * transport, eqs (33)-(35) PAPER.md:229-250 -- the flux kernels then also store a_+, a_- and the
  * upwind transverse velocities of every face on a 3-cell transverse apron, and the edges are
  * updated by their own kernel);
+ * "uct_passes" (1 default: the upwind-CT edges per reconstruction axis, each parabola once; 0: one
+ * thread per edge), "uct_nseg" (segments of the marching passes, default 16);
  * "c2p_backup" (1: when the 2-D Newton con2prim fails, try the 1-D scheme of PAPER.md:297-320,
  * eqs (42)-(45), before resetting the cell to atmosphere -- the paper's policy, PAPER.md:684;
  * 0 = off, the default: failure -> atmosphere, G20);
