@@ -111,97 +111,79 @@ __device__ __forceinline__ int uct_vbar_field(int a, int b) {  // vbar^a on the 
   return F_W + 4 * b + (a == (b + 1) % 3 ? 2 : 3);
 }
 
-// A = 1, 2: lanes along x, one thread per (i, t) column marching along A with the PPM state of
-// the four quantities carried in registers (FtMarch, as in the flux kernels).
+// A = 1, 2: lanes along x, one thread per (i, t) column and bracket (blockIdx.y = 2 t + w:
+// w = 0 the bracket br(A, A+1) -> -E_{A+2}, w = 1 br(A, A+2) -> +E_{A+1}) marching along A with
+// the PPM state of its two quantities carried in registers (FtMarch, as in the flux kernels).
+// `wr` bit w: this bracket is the first contribution (write), else add; `fin` bit w: it is the
+// last one -- the component goes straight into R11 + the RK combination.
 #ifndef UM_MINB
-#define UM_MINB 4
+#define UM_MINB 6
 #endif
 template <int A>
 __global__ void __launch_bounds__(128, UM_MINB)
 k_uct_march(double* __restrict__ base, Geom g, int seglen, int wr, int fin,
             const DevState* __restrict__ st, RkStage rk, int gauge) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int t = blockIdx.y;
+  const int t = blockIdx.y >> 1;
+  const int w = blockIdx.y & 1;
   if (i > g.nx) return;
   const int nA = g.n(A);
   const int m0 = (int)blockIdx.z * seglen, m1 = min(m0 + seglen, nA + 1);
-  constexpr int b1 = (A + 1) % 3, b2 = (A + 2) % 3;
-  constexpr int c1 = (A + 2) % 3, c2 = (A + 1) % 3;  // br1 -> -E_c1, br2 -> +E_c2
-  const long long sA = g.stride(A), s1 = g.stride(b1), s2 = g.stride(b2);
+  const int b = (A + 1 + w) % 3;     // the faces whose quantities are reconstructed along A
+  const int comp = (A + 2 - w) % 3;  // the edge component this bracket belongs to
+  const double sign = w ? 1.0 : -1.0;
+  const long long sA = g.stride(A), sb = g.stride(b);
   const long long c0 = A == 1 ? g.at(i, 0, t) : g.at(i, t, 0);  // position 0 along A
-  const double* q[4] = {fld(base, g, uct_vbar_field(A, b1)) + c0, fld(base, g, F_BF + b1) + c0,
-                        fld(base, g, uct_vbar_field(A, b2)) + c0, fld(base, g, F_BF + b2) + c0};
+  const double* q[2] = {fld(base, g, uct_vbar_field(A, b)) + c0, fld(base, g, F_BF + b) + c0};
   const double* Ap = fld(base, g, F_W + 4 * A) + c0;
   const double* Am = fld(base, g, F_W + 4 * A + 1) + c0;
-  double* E1 = uct_escratch(base, g, c1) + c0;
-  double* E2 = uct_escratch(base, g, c2) + c0;
-  // which of the two finished components exist at this (i, t): E_x for i < nx, else the index
-  // along the component's own axis (t is the index along b2 for A = 1, along b1 for A = 2)
-  const int tb = A == 1 ? 2 : 1;  // axis of t
-  const bool ok1 = c1 == 0 ? i < g.nx : (c1 == tb ? t < g.n(c1) : true);
-  const bool ok2 = c2 == 0 ? i < g.nx : (c2 == tb ? t < g.n(c2) : true);
+  double* Ec = uct_escratch(base, g, comp) + c0;
+  // does the component exist at this (i, t)?  E_x needs i < nx; otherwise the index along the
+  // component's own axis, which is t's axis here (comp != A)
+  const bool ok = comp == 0 ? i < g.nx : t < g.n(comp);
+  const bool first = (wr >> w) & 1, last = (fin >> w) & 1;
   const double h = st->dt;
   const double* GA = fld(base, g, F_GV) + c0;
-  FtMarch<1> mv[4];
+  const long long sc = g.stride(comp);
+  FtMarch<1> mv[2];
 #pragma unroll
-  for (int v = 0; v < 4; v++) {
+  for (int v = 0; v < 2; v++) {
     mv[v].init(q[v][(m0 - 3) * sA], q[v][(m0 - 2) * sA], q[v][(m0 - 1) * sA], q[v][m0 * sA]);
     double qm, qp;
     mv[v].step(q[v][(m0 + 1) * sA], 0.0, false, qm, qp);  // position m0 - 1
     mv[v].qpp = qp;
   }
   // values of the next step, loaded one step ahead
-  double nq[4], na[6];
+  double nq[2], na[4];
   auto fetch = [&](int m) {
     const long long c = m * sA;
-#pragma unroll
-    for (int v = 0; v < 4; v++) nq[v] = q[v][c + 2 * sA];
-    na[0] = Ap[c]; na[1] = Ap[c - s1]; na[2] = Ap[c - s2];
-    na[3] = Am[c]; na[4] = Am[c - s1]; na[5] = Am[c - s2];
+    nq[0] = q[0][c + 2 * sA]; nq[1] = q[1][c + 2 * sA];
+    na[0] = Ap[c]; na[1] = Ap[c - sb]; na[2] = Am[c]; na[3] = Am[c - sb];
   };
   fetch(m0);
   for (int m = m0; m < m1; m++) {
-    double cq[4], ca[6];
-#pragma unroll
-    for (int v = 0; v < 4; v++) cq[v] = nq[v];
-#pragma unroll
-    for (int v = 0; v < 6; v++) ca[v] = na[v];
+    const double cq0 = nq[0], cq1 = nq[1];
+    const double ap = ft_max(na[0], na[1]), am = ft_max(na[2], na[3]);
     if (m + 1 < m1) fetch(m + 1);
-    double L[4], R[4];
-#pragma unroll
-    for (int v = 0; v < 4; v++) {
+    double L[2], R[2];
+    {
       double qm, qp;
-      mv[v].step(cq[v], 0.0, false, qm, qp);
-      L[v] = mv[v].qpp;  // q^+ of position m - 1
-      R[v] = qm;         // q^- of position m
-      mv[v].qpp = qp;
+      mv[0].step(cq0, 0.0, false, qm, qp);
+      L[0] = mv[0].qpp; R[0] = qm; mv[0].qpp = qp;  // q^+ of position m-1, q^- of position m
+      mv[1].step(cq1, 0.0, false, qm, qp);
+      L[1] = mv[1].qpp; R[1] = qm; mv[1].qpp = qp;
     }
     const long long c = m * sA;
-    const double br1 = uct_combine(ft_max(ca[0], ca[1]), ft_max(ca[3], ca[4]), L[0], R[0], L[1],
-                                   R[1]);
-    const double br2 = uct_combine(ft_max(ca[0], ca[2]), ft_max(ca[3], ca[5]), L[2], R[2], L[3],
-                                   R[3]);
-    const double e1 = (wr & 1) ? -br1 : E1[c] - br1;
-    const double e2 = (wr & 2) ? br2 : E2[c] + br2;
-    // a component whose second bracket this is goes straight into R11 + RK (no second trip)
-    const bool in1 = ok1 && (c1 != A || m < nA), in2 = ok2 && (c2 != A || m < nA);
-    if (fin & 1) {
-      if (in1) {
-        double rhs = -e1;
-        if (gauge) rhs -= (GA[c + g.stride(c1)] - GA[c]) * g.idx[c1];
-        rk_apply(base, g, 5 + c1, c0 + c, rhs, h, rk);
+    const double br = sign * uct_combine(ap, am, L[0], R[0], L[1], R[1]);
+    const double e = first ? br : Ec[c] + br;
+    if (last) {
+      if (ok) {
+        double rhs = -e;
+        if (gauge) rhs -= (GA[c + sc] - GA[c]) * g.idx[comp];
+        rk_apply(base, g, 5 + comp, c0 + c, rhs, h, rk);
       }
     } else {
-      E1[c] = e1;
-    }
-    if (fin & 2) {
-      if (in2) {
-        double rhs = -e2;
-        if (gauge) rhs -= (GA[c + g.stride(c2)] - GA[c]) * g.idx[c2];
-        rk_apply(base, g, 5 + c2, c0 + c, rhs, h, rk);
-      }
-    } else {
-      E2[c] = e2;
+      Ec[c] = e;
     }
   }
 }

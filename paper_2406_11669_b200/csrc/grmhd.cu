@@ -529,10 +529,10 @@ int one_step(grmhd* h) {
         const int nsg = h->uct_nseg;
         const int sly = (g.ny + 1 + nsg - 1) / nsg, slz = (g.nz + 1 + nsg - 1) / nsg;
         // pass y finishes E_z, pass z finishes E_y and E_x: those go straight into R11 + RK
-        k_uct_march<1><<<dim3((g.nx + 1 + 127) / 128, g.nz + 1, (g.ny + sly) / sly), 128, 0,
+        k_uct_march<1><<<dim3((g.nx + 1 + 127) / 128, 2 * (g.nz + 1), (g.ny + sly) / sly), 128, 0,
                          h->s>>>(h->base, g, sly, 1, 2, h->dst, st[s], gauge);
         CKL("k_uct_march");
-        k_uct_march<2><<<dim3((g.nx + 1 + 127) / 128, g.ny + 1, (g.nz + slz) / slz), 128, 0,
+        k_uct_march<2><<<dim3((g.nx + 1 + 127) / 128, 2 * (g.ny + 1), (g.nz + slz) / slz), 128, 0,
                          h->s>>>(h->base, g, slz, 0, 3, h->dst, st[s], gauge);
         CKL("k_uct_march");
       } else if (h->E.emf) {
