@@ -154,6 +154,10 @@ int grmhd_get_psi(grmhd* h, double* field);
  * 0 = off, the default: failure -> atmosphere, G20);
  * "flux_kernel" (1 default: TMA-fed kernels; 0: the all-register marching kernel everywhere),
  * "flux_x_rows" (1 default: lanes-along-x kernel for the x fluxes; 0: as y and z);
+ * "graph" (1 default: after one eager step the launch sequence of a step is captured into a
+ * CUDA graph and every later step is one cudaGraphLaunch into the handle's stream -- same
+ * kernels, same arguments, bit-identical results; any other option or grmhd_set_mask drops the
+ * graph; bypassed while "kernel_timing" is on; 0: always launch kernel by kernel);
  * "kernel_timing" (1: bracket every kernel group of the step with CUDA events on the
  * handle's stream and accumulate device times, see grmhd_get_kernel_times; 0 = off;
  * setting it clears the accumulators).  Unknown key -> EINVAL. */

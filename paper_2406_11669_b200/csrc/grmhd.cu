@@ -44,6 +44,14 @@ struct grmhd {
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
   int xrow = 1;          // x fluxes: 1 k_flux_xrow (lanes along x), 0 as y and z
   int flux_impl = 1;     // 1: k_flux_tma (+ k_flux_march on the apron columns), 0: k_flux_march
+  // CUDA graph of one RK step (launch-bound small blocks): the first step after a change of
+  // options or mask runs eagerly (lazy attribute / occupancy queries happen there), the second
+  // is captured on cap_s, later ones are one cudaGraphLaunch into the caller's stream.
+  int use_graph = 1;
+  int gstate = 0;        // 0 nothing run yet, 1 eager step done, 2 graph ready, 3 capture failed
+  cudaStream_t cap_s = nullptr;
+  cudaGraphExec_t gexec = nullptr;
+  long long glaunches = 0;  // kernels per graph launch
   char err[256] = {0};
   // optional per-kernel-group timing ("kernel_timing" option): CUDA events on the stream
   bool ktime = false;
@@ -484,7 +492,7 @@ int compute_fluxes(grmhd* h) {
   return GRMHD_OK;
 }
 
-int one_step(grmhd* h) {
+int one_step_eager(grmhd* h) {
   const Geom& g = h->g;
   KT(KG_MISC, {
     k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 0);
@@ -550,6 +558,61 @@ int one_step(grmhd* h) {
   });
   h->steps++;
   return GRMHD_OK;
+}
+
+void graph_drop(grmhd* h) {
+  if (h->gexec) cudaGraphExecDestroy(h->gexec);
+  h->gexec = nullptr;
+  h->gstate = 0;
+}
+
+// Capture one_step_eager on the handle's own capture stream (the caller's stream may be the
+// legacy default stream, which cannot be captured).  Nothing executes during the capture.
+void graph_capture(grmhd* h) {
+  h->gstate = 3;
+  if (!h->cap_s && cudaStreamCreateWithFlags(&h->cap_s, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    h->cap_s = nullptr;
+    return;
+  }
+  cudaStream_t user = h->s;
+  const long long l0 = h->launches, s0 = h->steps;
+  if (cudaStreamBeginCapture(h->cap_s, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+    cudaGetLastError();
+    return;
+  }
+  h->s = h->cap_s;
+  const int rc = one_step_eager(h);
+  h->s = user;
+  cudaGraph_t gr = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(h->cap_s, &gr);
+  h->glaunches = h->launches - l0;
+  h->launches = l0;
+  h->steps = s0;
+  if (rc == GRMHD_OK && e == cudaSuccess && gr &&
+      cudaGraphInstantiate(&h->gexec, gr, 0) == cudaSuccess)
+    h->gstate = 2;
+  else {
+    cudaGetLastError();
+    h->gexec = nullptr;
+    h->err[0] = 0;
+  }
+  if (gr) cudaGraphDestroy(gr);
+}
+
+int one_step(grmhd* h) {
+  if (h->use_graph && !h->ktime) {
+    if (h->gstate == 1) graph_capture(h);
+    if (h->gstate == 2) {
+      CK(cudaGraphLaunch(h->gexec, h->s));
+      h->launches += h->glaunches;
+      h->steps++;
+      return GRMHD_OK;
+    }
+  }
+  const int rc = one_step_eager(h);
+  if (rc == GRMHD_OK && h->gstate == 0) h->gstate = 1;
+  return rc;
 }
 
 // field_from_potential + prim->cons + max speed
@@ -621,6 +684,8 @@ int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3], const g
 int grmhd_destroy(grmhd* h) {
   if (!h) return GRMHD_EINVAL;
   cudaStreamSynchronize(h->s);
+  graph_drop(h);
+  if (h->cap_s) cudaStreamDestroy(h->cap_s);
   for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
   delete h;
   return GRMHD_OK;
@@ -699,6 +764,7 @@ int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
 
 int grmhd_set_mask(grmhd* h, const unsigned char* mask) {
   if (!h) return GRMHD_EINVAL;
+  graph_drop(h);  // the mask pointer is a kernel argument
   if (!mask) { h->have_mask = false; return GRMHD_OK; }
   const Geom& g = h->g;
   const long long n = (long long)(g.nx + 2 * G) * (g.ny + 2 * G) * (g.nz + 2 * G);
@@ -798,6 +864,13 @@ int grmhd_get_psi(grmhd* h, double* field) {
 
 int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (!h || !key) return GRMHD_EINVAL;
+  if (std::strcmp(key, "graph") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: graph is 0 or 1");
+    h->use_graph = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "fixed_dt") != 0 && std::strcmp(key, "kernel_timing") != 0)
+    graph_drop(h);  // every other option changes kernel arguments or the launch sequence
   if (std::strcmp(key, "fixed_dt") == 0) {
     h->fixed_dt = value;
     return GRMHD_OK;

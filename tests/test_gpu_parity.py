@@ -379,6 +379,40 @@ def test_bns_100_substeps_smooth():
     _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL100, "bns 25 RK4 steps")
 
 
+def test_cuda_graph_step_is_bit_identical_to_eager():
+    """The captured step (third step on: one cudaGraphLaunch) runs the same kernels with the
+    same arguments as the eager path: bit-identical state, same launch count; an option change
+    drops the graph and the next steps use the new kernels."""
+    for w in (wl.balsara1(64, 4, 4), wl.c2p_stress(36)):
+        a, b = make_gpu(w), make_gpu(w)
+        a.set_option("graph", 0)
+        la, lb = a.launch_count(), b.launch_count()
+        a.step(6, w.cfl)
+        b.step(3, w.cfl)
+        b.step(3, w.cfl)
+        assert a.launch_count() - la == b.launch_count() - lb
+        for x, y in zip(to_np(a.get_cons()), to_np(b.get_cons())):
+            assert np.array_equal(x, y), w.name
+        sa, sb = a.stats(), b.stats()
+        assert sa["steps"] == sb["steps"] == 6 and sa["t"] == sb["t"] and sa["dt"] == sb["dt"]
+        # change the launch sequence after the capture: other x-flux kernel on both
+        a.set_option("flux_x_rows", 0)
+        b.set_option("flux_x_rows", 0)
+        a.step(4, w.cfl)
+        b.step(4, w.cfl)
+        for x, y in zip(to_np(a.get_cons()), to_np(b.get_cons())):
+            assert np.array_equal(x, y), w.name + " after set_option"
+        # new data on the same handle: the graph stays valid (same workspace, same arguments)
+        for s in (a, b):
+            s.set_prims(w.prims)
+            if w.vecpot is not None:
+                s.set_vecpot(w.vecpot)
+            s.step(2, w.cfl)
+        for x, y in zip(to_np(a.get_cons()), to_np(b.get_cons())):
+            assert np.array_equal(x, y), w.name + " after set_prims"
+        a.close(); b.close()
+
+
 def test_config1_full_run_to_t04():
     """Config 1 at full size and full length: same number of steps, same final state."""
     w = wl.balsara1(256, 4, 4)
