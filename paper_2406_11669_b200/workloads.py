@@ -393,7 +393,7 @@ def bns_like(n=512, seed=SEED0 + 4):
     k2 = np.maximum(kk * kk, 1.0)
     div = (KX * specs[0] + KY * specs[1] + KZ * specs[2]) / k2
     specs = [specs[0] - KX * div, specs[1] - KY * div, specs[2] - KZ * div]
-    u = [np.fft.irfftn(s, s=(n, n, n)) for s in specs]
+    u = [np.fft.irfftn(s, s=(n, n, n), axes=(0, 1, 2)) for s in specs]
     rms = np.sqrt(np.mean(u[0] ** 2 + u[1] ** 2 + u[2] ** 2))
     v = [0.5 * cs * c / rms for c in u]
     v2 = psi4 * (v[0] ** 2 + v[1] ** 2 + v[2] ** 2)
@@ -404,7 +404,7 @@ def bns_like(n=512, seed=SEED0 + 4):
     A = []
     for sh in shifts:
         s, _ = _random_spectrum_field(rng, n, -17.0 / 6.0, kmax, sh)
-        A.append(np.fft.irfftn(s, s=(n, n, n)))
+        A.append(np.fft.irfftn(s, s=(n, n, n), axes=(0, 1, 2)))
     zero = np.zeros_like(U)
     metric_int = [alpha, zero, zero, zero, psi4, zero, zero, psi4, zero, psi4,
                   zero, zero, zero, zero, zero, zero]
