@@ -243,8 +243,18 @@ int zero_field(grmhd* h, int id) {
 }
 
 // R15: x, then y, then z pass
+constexpr long long FILL_FUSE_MAX = 1LL << 20;  // padded cells: below, launches cost more than threads
+
 int fill_ghosts(grmhd* h, const FillArgs& fa) {
   const Geom& g = h->g;
+  bool plain = true;  // unstaggered copy / wrap fields only
+  for (int f = 0; f < fa.nf; f++) plain = plain && fa.stag[f] == 0 && fa.kind[f] == 0;
+  const long long npad = (long long)(g.nx + 2 * G) * (g.ny + 2 * G) * (g.nz + 2 * G);
+  if (plain && npad <= FILL_FUSE_MAX) {
+    k_fill_copy3<<<dim3((unsigned)((npad + 255) / 256), 1, fa.nf), 256, 0, h->s>>>(h->base, g, fa);
+    CKL("k_fill_copy3");
+    return GRMHD_OK;
+  }
   for (int a = 0; a < 3; a++) {
     const int b0 = (a + 1) % 3, b1 = (a + 2) % 3;
     const long long nt = (long long)(g.n(b0) + 2 * G + 1) * (g.n(b1) + 2 * G + 1);

@@ -153,6 +153,28 @@ __global__ void k_fill_axis(double* __restrict__ base, Geom g, FillArgs fa, int 
   }
 }
 
+// R15 for unstaggered copy / wrap fields (the primitives) in one launch: the x, y, z passes of
+// k_fill_axis compose to one index map per axis (wrap with period n, or clamp to the nearest
+// interior cell), so every ghost cell reads its interior source directly -- bit-identical, and
+// two launches fewer per substep on blocks that are launch bound.  One thread per padded cell.
+__global__ void k_fill_copy3(double* __restrict__ base, Geom g, FillArgs fa) {
+  const int W0 = g.nx + 2 * G, W1 = g.ny + 2 * G, W2 = g.nz + 2 * G;
+  const long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (tid >= (long long)W0 * W1 * W2) return;
+  const int i = (int)(tid % W0) - G, j = (int)((tid / W0) % W1) - G;
+  const int k = (int)(tid / ((long long)W0 * W1)) - G;
+  if (i >= 0 && i < g.nx && j >= 0 && j < g.ny && k >= 0 && k < g.nz) return;
+  const int I[3] = {i, j, k};
+  int S[3];
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const int n = g.n(a);
+    S[a] = g.bc[a] == 0 ? ((I[a] % n) + n) % n : min(max(I[a], 0), n - 1);
+  }
+  double* q = fld(base, g, fa.id[blockIdx.z]);
+  q[g.at(i, j, k)] = q[g.at(S[0], S[1], S[2])];
+}
+
 // --------------------------------------------------------------------------- B from A
 // R13: B~^i = B~0^i + [ijk] d_j A_k on faces (eq. 24 PAPER.md:149 with
 // epsilon^{ijk} = [ijk]/sqrt(gamma)), then the cell-centre value as the mean
