@@ -152,8 +152,9 @@ int grmhd_get_psi(grmhd* h, double* field);
  * "c2p_backup" (1: when the 2-D Newton con2prim fails, try the 1-D scheme of PAPER.md:297-320,
  * eqs (42)-(45), before resetting the cell to atmosphere -- the paper's policy, PAPER.md:684;
  * 0 = off, the default: failure -> atmosphere, G20);
- * "flux_kernel" (1 default: TMA-fed kernels; 0: the all-register marching kernel everywhere),
- * "flux_x_rows" (1 default: lanes-along-x kernel for the x fluxes; 0: as y and z);
+ * "flux_kernel" (1 default: y and z fluxes by the TMA-fed marching kernel, x fluxes with the lanes
+ * of a warp along x; 0: lanes along the flux direction in all three directions -- what blocks
+ * narrower than 32 cells in x use anyway);
  * "graph" (1 default: after one eager step the launch sequence of a step is captured into a
  * CUDA graph and every later step is one cudaGraphLaunch into the handle's stream -- same
  * kernels, same arguments, bit-identical results; any other option or grmhd_set_mask drops the

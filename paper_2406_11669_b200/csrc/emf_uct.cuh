@@ -1,7 +1,6 @@
 // emf_uct.cuh -- row F1: the electric field on the edges by the upwind constrained transport
 // (eqs 33-35; readings G26-G28 of DESIGN.md) and the update of A_i.
 #pragma once
-#include "flux_tma.cuh"
 #include "flux_xrow.cuh"
 #include "kernels_flux.cuh"
 
@@ -14,7 +13,7 @@ namespace gk {
 // flattening: L from the lower, R from the upper side), combined with the larger a_+, a_- of
 // the two a-faces that share the edge.  c = index of the edge, sa / sb = strides of a and b.
 // G8 without flattening on the 6 values s[0..5] around a position: L = q^+ of cell 2, R = q^- of
-// cell 3; branch free, same arithmetic as FtMarch::step.
+// cell 3; branch free, same arithmetic as FtMarch::step (flux_face.cuh).
 // monotonised q^+ (UPPER = true) or q^- of a cell from its two interface values
 template <bool UPPER>
 __device__ __forceinline__ double uct_limit(double q, double qm, double qp) {
@@ -95,7 +94,7 @@ k_emf_uct(double* __restrict__ base, Geom g, const DevState* __restrict__ st, Rk
 //   br(A, A+1) -> -E_{A+2},   br(A, A+2) -> +E_{A+1}
 // into three scratch fields (the flux-CT B rows F_FX+5, F_FY+5, F_FZ+5, unused with the upwind
 // CT, hold E_x, E_y, E_z).  Pass order x, y, z; `wr` bit 0 / bit 1 = the first / second
-// bracket writes (first contribution) instead of adding.  k_emf_apply then does R11 + RK.
+// bracket writes (first contribution) instead of adding; the last one goes into R11 + RK.
 __device__ __forceinline__ double* uct_escratch(double* base, const Geom& g, int comp) {
   return fld(base, g, comp == 0 ? F_FX + 5 : (comp == 1 ? F_FY + 5 : F_FZ + 5));
 }
@@ -224,25 +223,6 @@ k_uct_xrow(double* __restrict__ base, Geom g, int nsd, long long nitems, int wr)
     E1[c] = (wr & 1) ? -br1 : E1[c] - br1;
     E2[c] = (wr & 2) ? br2 : E2[c] + br2;
   }
-}
-
-// R11 + RK on the edges from the scratch E (one thread per edge: blockIdx.z = 3 k + comp)
-__global__ void __launch_bounds__(256)
-k_emf_apply(double* __restrict__ base, Geom g, const DevState* __restrict__ st, RkStage rk,
-            int gauge) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z / 3;
-  const int comp = blockIdx.z % 3;
-  if (i > g.nx || j > g.ny) return;
-  if ((comp == 0 && i >= g.nx) || (comp == 1 && j >= g.ny) || (comp == 2 && k >= g.nz)) return;
-  const long long c = g.at(i, j, k);
-  double rhs = -uct_escratch(base, g, comp)[c];
-  if (gauge) {  // eq. (31): - d_comp G_A
-    const double* GA = fld(base, g, F_GV);
-    rhs -= (GA[c + g.stride(comp)] - GA[c]) * g.idx[comp];
-  }
-  rk_apply(base, g, 5 + comp, c, rhs, st->dt, rk);
 }
 
 // ------------------------------------------------------------ generalised Lorenz gauge

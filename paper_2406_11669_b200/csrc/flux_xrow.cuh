@@ -1,9 +1,8 @@
 // flux_xrow.cuh -- A3 + A4 along x with the lanes of a warp ALONG x.
 //
-// x is the contiguous axis: a kernel that marches along x (flux_tma.cuh, D = 0) can only
-// touch 32 bytes of a row at a time, which HBM serves badly (ncu capture r1g: the prefetched
-// cells arrive late, DRAM reads 1.45x the algorithmic bytes).  Here a warp owns 32 consecutive
-// cells c0 .. c0+31 of one row (j, k); lane = cell.  Every load and store is a contiguous
+// x is the contiguous axis: a kernel that marches along x can only touch 32 bytes of a row at
+// a time, which HBM serves badly (measured in round 1: 1.45x DRAM over-fetch, 1.7 ms against
+// 1.0 ms).  Here a warp owns 32 consecutive cells c0 .. c0+31 of one row (j, k); lane = cell.  Every load and store is a contiguous
 // 256-byte row segment.  The reconstruction recurrences run across lanes: the limited slope,
 // the interface value and the parabola of a cell are computed once, by the cell's lane, and
 // handed to the neighbour with warp shuffles (R5/G8: slope of c+1 from the lane above,
@@ -12,7 +11,7 @@
 // a warp yields 27 faces; consecutive warps overlap by 5 cells.  No shared memory, no block
 // barrier, nothing carried from one row segment to the next.
 #pragma once
-#include "flux_tma.cuh"
+#include "flux_face.cuh"
 
 namespace gk {
 
@@ -43,23 +42,9 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
     const double dm = ft_slope(dl, dr);
     const double dmp = fx_dn(dm, 1);                             // slope of cell c+1
     const double ir = 0.5 * (q + qp1) - (dmp - dm) * (1.0 / 6.0);  // interface c + 1/2
-    const double il = fx_up(ir, 1);                              // interface c - 1/2
-    qm = il; qp = ir;
-    if (RECON == 2 && anyf) {
-      const double qpf = f * q + (1.0 - f) * qp;
-      const double qmf = f * q + (1.0 - f) * qm;
-      qp = f != 0.0 ? qpf : qp;
-      qm = f != 0.0 ? qmf : qm;
-    }
-    const double a = qp - q, b = q - qm;
-    const double aa = fabs(a), ab = fabs(b);
-    const bool flat = ft_opposite(a, b);
-    const bool fixm = ab > 2.0 * aa;
-    const bool fixp = aa > 2.0 * ab;
-    const double qm2 = fma(-2.0, a, q);
-    const double qp2 = fma(2.0, b, q);
-    qm = ft_sel(flat, q, ft_sel(fixm, qm2, qm));
-    qp = ft_sel(flat, q, ft_sel(fixp, qp2, qp));
+    qm = fx_up(ir, 1);                                           // interface c - 1/2
+    qp = ir;
+    ft_parabola<RECON == 2>(q, f, anyf, qm, qp);
   }
 }
 
@@ -81,7 +66,6 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
   const int nD = g.n(D);
   const int nt0 = D == 0 ? g.ny : g.nx;
   const int w0 = mode ? 2 * ap : nt0 + 2 * ap;
-  const int sd = D == 0 ? 1 : (D == 1 ? (int)g.sy : (int)g.sz);
   // grid-stride loop over the items (the launch gives every warp one item)
   for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
        item < nitems; item += nwarp) {
@@ -93,75 +77,48 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
   const int t0 = mode ? (q0 < ap ? q0 - ap : nt0 + q0 - ap) : q0 - ap;
   const int idx = (int)(D == 0 ? g.at(cc, t0, t1) : (D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc)));
 
-  // ---- cell data of the lane: rho, v^x, v^y, v^z, p, B^y, B^z
-  double q[FM_NV];
+  // ---- cell data of the lane: rho, v^x, v^y, v^z, p and the two transverse B; the static face
+  // metric and the staggered normal field of the lane's face c - 1/2
+  double q[FX_NV];
 #pragma unroll
-  for (int v = 0; v < FM_NV; v++) q[v] = fld(base, g, fm_var_field(D, v))[idx];
+  for (int v = 0; v < FX_NV; v++) q[v] = fld(base, g, flux_var_field(D, v))[idx];
   const double bfx = fld(base, g, F_BF + D)[idx];
-  // ---- face metric (R4): 4-point Lagrange along D.  Lanes 0-2 have no face to solve: their
-  // stencil base is moved to cell -1 so that it stays inside the padded array.
-  const int idxm = idx + (max(cc, -1) - cc) * sd;
-  Met M;
-  {
-    double mq[FT_NMET];
+  double mv11[NFM];
 #pragma unroll
-    for (int v = 0; v < FT_NMET; v++) {
-      const double* m = fld(base, g, F_MET + v) + idxm;
-      mq[v] = (-m[-2 * sd] + 9.0 * m[-sd] + 9.0 * m[0] - m[sd]) * 0.0625;
-    }
-    M.a = mq[0]; M.bx = mq[1]; M.by = mq[2]; M.bz = mq[3];
-    M.gxx = mq[4]; M.gxy = mq[5]; M.gxz = mq[6]; M.gyy = mq[7]; M.gyz = mq[8]; M.gzz = mq[9];
-  }
+  for (int v = 0; v < NFM; v++) mv11[v] = fld(base, g, F_FM + NFM * D + v)[idx];
   // ---- neighbours across lanes
-  double qm1[FM_NV], qp1[FM_NV];
+  double qm1[FX_NV], qp1[FX_NV];
 #pragma unroll
-  for (int v = 0; v < FM_NV; v++) { qm1[v] = fx_up(q[v], 1); qp1[v] = fx_dn(q[v], 1); }
+  for (int v = 0; v < FX_NV; v++) { qm1[v] = fx_up(q[v], 1); qp1[v] = fx_dn(q[v], 1); }
   // G8(c): flattening coefficient of the lane's cell from p_{c-2..c+2}, v^D_{c-1}, v^D_{c+1}
   double f = 0.0;
   bool anyf = false;
   if (RECON == 2) {
-    const double pm2 = fx_up(q[4], 2), pp2 = fx_dn(q[4], 2);
-    const double dp1 = qp1[4] - qm1[4];
-    const double dp2 = pp2 - pm2;
-    const bool on = fabs(dp1) > 0.33 * ft_min(qp1[4], qm1[4]) && qm1[1 + D] > qp1[1 + D];
-    const bool z = dp2 == 0.0;
-    const double r = ft_rcp(z ? 1.0 : dp2);
-    double ff = 10.0 * fma(dp1, r, -0.75);
-    ff = ft_min(1.0, ft_max(0.0, ff));
-    ff = z ? 1.0 : ff;
-    f = on ? ff : 0.0;
+    f = ft_flatten(fx_up(q[4], 2), qm1[4], qp1[4], fx_dn(q[4], 2), qm1[1 + D], qp1[1 + D]);
     anyf = __any_sync(0xffffffffu, f != 0.0);
   }
-  double qL[FM_NV], qR[FM_NV];
+  double qL[FX_NV], qR[FX_NV];
 #pragma unroll
-  for (int v = 0; v < FM_NV; v++) {
+  for (int v = 0; v < FX_NV; v++) {
     double qm, qp;
     fx_recon<RECON>(q[v], qm1[v], qp1[v], f, anyf, qm, qp);
     qL[v] = fx_up(qp, 1);  // q^+ of cell c-1
     qR[v] = qm;
   }
   // ---- Riemann problem of face c - 1/2 (R7)
-  const double det = det_gamma(M);
-  const double isg = ft_rsqrt(det);
-  const double sgf = det * isg;
-  const double gdd = inv_gamma_dd<D>(M, isg * isg);
-  const double Bn = bfx * isg;  // G6
-  double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR, vtL[2], vtR[2], apm[2];
-  // slots 5, 6 hold B^{(D+1)%3}, B^{(D+2)%3}
-  ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
-             D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]), M,
-             gdd, E, UL, GL, lmL, lpL, UCT ? vtL : nullptr);
-  ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
-             D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]), M,
-             gdd, E, UR, GR, lmR, lpR, UCT ? vtR : nullptr);
-  double out[7];
-  ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, sgf, E.riemann, out, UCT ? apm : nullptr);
+  const FaceMet fmet = face_met<D>(mv11);
+  double out[7], w[4];
+  ft_face<D, UCT>(qL, qR, bfx, fmet, E, out, w);
   if (lane >= 3 && lane < 3 + FX_VALID && c <= nD) {
-    double* o = fld(base, g, D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ)) + idx;
+    double* o = fld(base, g, flux_field(D)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
     for (int r = 0; r < 7; r++) o[r * NPA] = out[r];
-    if (UCT) ft_store_uct(fld(base, g, F_W + 4 * D) + idx, NPA, apm, vtL, vtR);
+    if (UCT) {
+      double* ow = fld(base, g, F_W + 4 * D) + idx;
+#pragma unroll
+      for (int r = 0; r < 4; r++) ow[r * NPA] = w[r];
+    }
   }
   }  // items
 }

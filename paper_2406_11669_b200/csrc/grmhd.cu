@@ -11,7 +11,6 @@
 #include <vector>
 
 #include "kernels_flux.cuh"
-#include "flux_march.cuh"
 #include "flux_tma.cuh"
 #include "flux_xrow.cuh"
 #include "emf_uct.cuh"
@@ -36,14 +35,13 @@ struct grmhd {
   double cfl_set = -1.0, fixed_dt = 0.0, fixed_set = -1.0, tend_set = -2.0;
   long long steps = 0;
   long long launches = 0;
-  int fm_conc[9] = {0};  // resident blocks of each flux-kernel instantiation (0 = not queried)
-  int ft_conc[18] = {0};  // ... of the TMA-fed instantiations
-  CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][.] of the ring stages, per direction
+  int ft_conc[18] = {0};  // resident blocks of each k_flux_tma instantiation (0 = not queried)
+  CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][x] of the ring stages (y, z)
   bool tma_ok = false;
   int uct_nseg = 16;     // segments of the marching passes along y and z
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
-  int xrow = 1;          // x fluxes: 1 k_flux_xrow (lanes along x), 0 as y and z
-  int flux_impl = 1;     // 1: k_flux_tma (+ k_flux_march on the apron columns), 0: k_flux_march
+  int flux_impl = 1;     // 1: y and z fluxes by k_flux_tma (blocks at least 32 cells wide in x),
+                         // 0: k_flux_xrow (lanes along the flux direction) everywhere
   // CUDA graph of one RK step (launch-bound small blocks): the first step after a change of
   // options or mask runs eagerly (lazy attribute / occupancy queries happen there), the second
   // is captured on cap_s, later ones are one cudaGraphLaunch into the caller's stream.
@@ -136,6 +134,7 @@ bool valid_opts(const grmhd_opts* o) {
     if (o->bc[a] != 0 && o->bc[a] != 1) return false;
   return o->rk >= 2 && o->rk <= 4 && o->recon >= 0 && o->recon <= 1 && o->gamma_ad > 1.0 &&
          o->p_floor > 0 && o->rho_atm > 0 && o->w_max > 1.0 && o->c2p_maxit >= 1 &&
+         o->c2p_tol > 0 && o->poly_k >= 0 && o->poly_gamma > 0 &&
          o->riemann >= 0 && o->riemann <= 1;
 }
 
@@ -192,6 +191,14 @@ bool is_device_ptr(const void* p) {
     return false;
   }
   return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// set_* calls stage host sources through cudaMemcpyAsync: wait for the copies before
+// returning, so that the caller may reuse or free its host arrays at once (device sources stay
+// asynchronous on the handle's stream)
+int sync_if_host(grmhd* h, const void* p) {
+  if (p && !is_device_ptr(p)) CK(cudaStreamSynchronize(h->s));
+  return GRMHD_OK;
 }
 
 dim3 blk3() { return dim3(32, 4, 1); }
@@ -320,44 +327,6 @@ int after_stage(grmhd* h, bool want_speed) {
   return GRMHD_OK;
 }
 
-// ---- marching flux kernel launch (flux_march.cuh) ----------------------------------------
-constexpr int FM_TC = 4;
-
-template <int D, int RECON>
-int launch_flux(grmhd* h, int apron) {
-  const Geom& g = h->g;
-  auto kern = k_flux_march<D, RECON, FM_TC>;
-  const int smem = (int)sizeof(FluxSmem<D, FM_TC>);
-  const int cfg = D * 3 + RECON;
-  if (h->fm_conc[cfg] == 0) {  // first use: opt in to the shared memory, query residency
-    CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    int nb = 0, dev = 0, nsm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, FM_THREADS, smem));
-    CK(cudaGetDevice(&dev));
-    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    h->fm_conc[cfg] = nb * nsm > 0 ? nb * nsm : 1;
-  }
-  const int nfaces = g.n(D) + 1;
-  const int ngroups = (fm_npencils(g, D, apron) + 31) / 32;
-  // segments along D: fill whole waves of resident blocks; a segment costs ~2 extra cells
-  int best = 1;
-  double best_cost = 1e300;
-  for (int ns = 1; ns <= 64; ns++) {
-    const int sl = ((nfaces + ns - 1) / ns + FM_TC - 1) / FM_TC * FM_TC;
-    if (ns > 1 && sl < 16) break;
-    const int nseg = (nfaces + sl - 1) / sl;
-    const long long nblk = (long long)nseg * ngroups;
-    const long long waves = (nblk + h->fm_conc[cfg] - 1) / h->fm_conc[cfg];
-    const double cost = (double)waves * (sl + 2);
-    if (cost < best_cost * 0.97) { best_cost = cost; best = ns; }
-  }
-  const int seglen = ((nfaces + best - 1) / best + FM_TC - 1) / FM_TC * FM_TC;
-  const int nseg = (nfaces + seglen - 1) / seglen;
-  kern<<<dim3(ngroups, nseg), FM_THREADS, smem, h->s>>>(h->base, g, h->E, seglen, apron);
-  h->launches++;
-  return GRMHD_OK;
-}
-
 // lanes along D (flux_xrow.cuh): one warp per 27 faces of a pencil.  mode 0: every pencil
 // (the x fluxes; any direction of a narrow block when the upwind CT is on); mode 1: the
 // apron columns k_flux_tma leaves out.
@@ -383,9 +352,6 @@ int launch_flux_xrow(grmhd* h, int mode) {
 }
 
 // ---- TMA-fed flux kernel (flux_tma.cuh) ---------------------------------------------------
-#ifndef FT_PROMO_X
-#define FT_PROMO_X CU_TENSOR_MAP_L2_PROMOTION_L2_256B
-#endif
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -406,17 +372,15 @@ bool make_tensor_maps(grmhd* h) {
   const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8,
                                  (cuuint64_t)g.NPA * 8};
   const cuuint32_t es[4] = {1, 1, 1, 1};
-  for (int d = 0; d < 3; d++) {
+  for (int d = 1; d < 3; d++) {
     for (int w = 0; w < 2; w++) {
-      cuuint32_t box[4] = {32, 1, 1, (cuuint32_t)(w == 0 ? FT_NMET : 1)};
-      if (d == 0) { box[0] = FT_TC; box[1] = 32; }
-      else box[d] = FT_TC;
+      cuuint32_t box[4] = {32, 1, 1, (cuuint32_t)(w == 0 ? NFM : 1)};
+      box[d] = FT_TC;
       CUresult r = ((EncodeTiledFn)fn)(w == 0 ? &h->tm_met[d] : &h->tm_bf[d],
                                        CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, h->base, dims, strides,
                                        box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                        CU_TENSOR_MAP_SWIZZLE_NONE,
-                                       d == 0 ? (CUtensorMapL2promotion)FT_PROMO_X
-                                              : CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
       if (r != CUDA_SUCCESS) return false;
     }
@@ -428,7 +392,7 @@ template <int D, int RECON, bool UCT>
 int launch_flux_tma_v(grmhd* h) {
   const Geom& g = h->g;
   auto kern = k_flux_tma<D, RECON, UCT>;
-  const int smem = (int)sizeof(FtSmem<D>);
+  const int smem = (int)sizeof(FtSmem);
   const int cfg = (UCT ? 9 : 0) + D * 3 + RECON;
   if (h->ft_conc[cfg] == 0) {
     CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -438,11 +402,11 @@ int launch_flux_tma_v(grmhd* h) {
     CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
     h->ft_conc[cfg] = nb * nsm > 0 ? nb * nsm : 1;
   }
-  const int nt0 = D == 0 ? g.ny : g.nx, nt1 = D == 2 ? g.ny : g.nz;
-  const int ngx = (nt0 + 31) / 32;
+  const int nt1 = D == 2 ? g.ny : g.nz;
+  const int ngx = (g.nx + 31) / 32;
   const int ap = apron_width(h);
   const long long ngroups = (long long)ngx * (nt1 + 2 * ap);
-  const int nfaces = g.n(D) + 1 + (D == 0 ? 2 : 0);  // D = x marches from face -2 (alignment)
+  const int nfaces = g.n(D) + 1;
   int best = 1;
   double best_cost = 1e300;
   for (int ns = 1; ns <= 64; ns++) {
@@ -461,9 +425,7 @@ int launch_flux_tma_v(grmhd* h) {
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_tma");
-  // the apron columns along t0 (the marching kernel only knows the 1-cell apron)
-  if ((D != 0 && h->xrow) || h->E.emf) return launch_flux_xrow<D, RECON>(h, 1);
-  return launch_flux<D, RECON>(h, 1);
+  return launch_flux_xrow<D, RECON>(h, 1);  // the apron columns along x
 }
 
 template <int D, int RECON>
@@ -471,26 +433,22 @@ int launch_flux_tma(grmhd* h) {
   return h->E.emf ? launch_flux_tma_v<D, RECON, true>(h) : launch_flux_tma_v<D, RECON, false>(h);
 }
 
+template <int D, int RECON>
+int launch_flux_dr(grmhd* h) {
+  if (D != 0 && h->flux_impl == 1 && h->tma_ok && h->g.nx >= 32) {
+    if constexpr (D != 0) return launch_flux_tma<D, RECON>(h);
+  }
+  return launch_flux_xrow<D, RECON>(h, 0);
+}
+
 template <int D>
 int launch_flux_d(grmhd* h) {
   const int recon = h->o.recon == 0 ? 0 : (h->o.ppm_flatten ? 2 : 1);
-  const int nt0 = D == 0 ? h->g.ny : h->g.nx;
-  int rc;
-  if (D == 0 && h->flux_impl == 1 && h->xrow)
-    rc = recon == 0 ? launch_flux_xrow<0, 0>(h, 0)
-                    : (recon == 1 ? launch_flux_xrow<0, 1>(h, 0) : launch_flux_xrow<0, 2>(h, 0));
-  else if (h->flux_impl == 1 && h->tma_ok && nt0 >= 32)
-    rc = recon == 0 ? launch_flux_tma<D, 0>(h)
-                    : (recon == 1 ? launch_flux_tma<D, 1>(h) : launch_flux_tma<D, 2>(h));
-  else if (h->E.emf)  // the marching kernel has neither the 3-cell apron nor the UCT face rows
-    rc = recon == 0 ? launch_flux_xrow<D, 0>(h, 0)
-                    : (recon == 1 ? launch_flux_xrow<D, 1>(h, 0) : launch_flux_xrow<D, 2>(h, 0));
-  else
-    rc = recon == 0 ? launch_flux<D, 0>(h, 0)
-                    : (recon == 1 ? launch_flux<D, 1>(h, 0) : launch_flux<D, 2>(h, 0));
+  const int rc = recon == 0 ? launch_flux_dr<D, 0>(h)
+                            : (recon == 1 ? launch_flux_dr<D, 1>(h) : launch_flux_dr<D, 2>(h));
   if (rc) return rc;
   cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_march");
+  if (e != cudaSuccess) return cuda_fail(h, e, "flux kernel");
   return GRMHD_OK;
 }
 
@@ -710,8 +668,19 @@ int grmhd_set_metric(grmhd* h, const double* const field[16]) {
     int rc = copy_in(h, field[f], F_MET + f, false);
     if (rc) return rc;
   }
+  // the metric is held fixed from here on: face values (R4) and sqrt(gamma_f) once
+  const dim3 fb(32, 4, 1), fg((h->g.PXP + 31) / 32, (h->g.PY + 3) / 4, h->g.PZ);
+  k_face_metric<0><<<fg, fb, 0, h->s>>>(h->base, h->g);
+  CKL("k_face_metric");
+  k_face_metric<1><<<fg, fb, 0, h->s>>>(h->base, h->g);
+  CKL("k_face_metric");
+  k_face_metric<2><<<fg, fb, 0, h->s>>>(h->base, h->g);
+  CKL("k_face_metric");
   h->have_metric = true;
-  return GRMHD_OK;
+  // a new metric under existing primitives: U~, B_c, the sources and the max speed are rebuilt
+  // from the primitives by the next call that needs them
+  if (h->have_prims) h->dirty = true;
+  return sync_if_host(h, field[0]);
 }
 
 int grmhd_set_prims(grmhd* h, const double* const field[8]) {
@@ -755,7 +724,7 @@ int grmhd_set_prims(grmhd* h, const double* const field[8]) {
   k_reset_state<<<1, 1, 0, h->s>>>(h->dst, 1);
   CKL("k_reset_state");
   h->dirty = true;
-  return GRMHD_OK;
+  return sync_if_host(h, field[0]);
 }
 
 int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
@@ -769,7 +738,7 @@ int grmhd_set_vecpot(grmhd* h, const double* const field[3]) {
     if (rc) return rc;
   }
   h->dirty = true;
-  return GRMHD_OK;
+  return sync_if_host(h, field[0]);
 }
 
 int grmhd_set_mask(grmhd* h, const unsigned char* mask) {
@@ -786,7 +755,7 @@ int grmhd_set_mask(grmhd* h, const unsigned char* mask) {
   k_repack_mask<<<grd1(n), 256, 0, h->s>>>(src, h->mask, g);
   CKL("k_repack_mask");
   h->have_mask = true;
-  return GRMHD_OK;
+  return sync_if_host(h, mask);
 }
 
 int grmhd_step(grmhd* h, int n, double cfl) {
@@ -917,11 +886,6 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   }
   if (std::strcmp(key, "uct_passes") == 0) {
     h->uct_passes = value != 0.0;
-    return GRMHD_OK;
-  }
-  if (std::strcmp(key, "flux_x_rows") == 0) {
-    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_x_rows is 0 or 1");
-    h->xrow = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "kernel_timing") == 0) {

@@ -175,6 +175,42 @@ __global__ void k_fill_copy3(double* __restrict__ base, Geom g, FillArgs fa) {
   q[g.at(i, j, k)] = q[g.at(S[0], S[1], S[2])];
 }
 
+// ------------------------------------------------------------------ static face metric
+// R4 (adapted per G3), once per grmhd_set_metric since the ADM variables are held
+// fixed: for the lower D-face of every padded index, the 4-point Lagrange values
+// q_f = (-q_{i-2} + 9 q_{i-1} + 9 q_i - q_{i+1})/16 of alpha, beta^k, gamma_kl along D and
+// sqrt(det gamma_f) -> field family F_FM + NFM D.  Faces whose stencil leaves the cells the
+// caller supplied (i_D outside [-1, n_D + 1], or a transverse index outside [-G, n + G)) take
+// the value of the nearest face inside: never used by a stored flux, but finite.
+template <int D>
+__global__ void __launch_bounds__(128)
+k_face_metric(double* __restrict__ base, Geom g) {
+  const int ix = blockIdx.x * blockDim.x + threadIdx.x;
+  const int iy = blockIdx.y * blockDim.y + threadIdx.y;
+  const int iz = blockIdx.z;
+  if (ix >= g.PXP || iy >= g.PY) return;
+  const long long dst = (long long)iz * g.sz + (long long)iy * g.sy + ix;
+  int I[3] = {ix - X0, iy - G, iz - G};
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    const int lo = a == D ? -1 : -G, hi = a == D ? g.n(a) + 1 : g.n(a) + G - 1;
+    I[a] = min(max(I[a], lo), hi);
+  }
+  const long long c = g.at(I[0], I[1], I[2]);
+  const long long sd = g.stride(D);
+  double m[10];
+#pragma unroll
+  for (int v = 0; v < 10; v++) {
+    const double* q = fld(base, g, F_MET + v);
+    m[v] = (-q[c - 2 * sd] + 9.0 * q[c - sd] + 9.0 * q[c] - q[c + sd]) * 0.0625;
+    fld(base, g, F_FM + NFM * D + v)[dst] = m[v];
+  }
+  Met M;
+  M.a = m[0]; M.bx = m[1]; M.by = m[2]; M.bz = m[3];
+  M.gxx = m[4]; M.gxy = m[5]; M.gxz = m[6]; M.gyy = m[7]; M.gyz = m[8]; M.gzz = m[9];
+  fld(base, g, F_FM + NFM * D + 10)[dst] = sqrt(det_gamma(M));
+}
+
 // --------------------------------------------------------------------------- B from A
 // R13: B~^i = B~0^i + [ijk] d_j A_k on faces (eq. 24 PAPER.md:149 with
 // epsilon^{ijk} = [ijk]/sqrt(gamma)), then the cell-centre value as the mean
@@ -191,33 +227,6 @@ __device__ __forceinline__ double face_by(const double* Ax, const double* Az, co
 __device__ __forceinline__ double face_bz(const double* Ax, const double* Ay, const double* B0z,
                                           const Geom& g, long long c) {
   return B0z[c] + (Ay[c + 1] - Ay[c]) * g.idx[0] - (Ax[c + g.sy] - Ax[c]) * g.idx[1];
-}
-
-__global__ void k_bfield(double* __restrict__ base, Geom g) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x - G;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y - G;
-  const int k = blockIdx.z - G;
-  if (i > g.nx + G || j > g.ny + G) return;
-  const long long c = g.at(i, j, k);
-  const double* Ax = fld(base, g, F_Y + 5);
-  const double* Ay = fld(base, g, F_Y + 6);
-  const double* Az = fld(base, g, F_Y + 7);
-  const double* B0x = fld(base, g, F_B0 + 0);
-  const double* B0y = fld(base, g, F_B0 + 1);
-  const double* B0z = fld(base, g, F_B0 + 2);
-  const bool ix = i < g.nx + G, jy = j < g.ny + G, kz = k < g.nz + G;
-  const double bx = (jy && kz) ? face_bx(Ay, Az, B0x, g, c) : B0x[c];
-  const double by = (ix && kz) ? face_by(Ax, Az, B0y, g, c) : B0y[c];
-  const double bz = (ix && jy) ? face_bz(Ax, Ay, B0z, g, c) : B0z[c];
-  fld(base, g, F_BF + 0)[c] = bx;
-  fld(base, g, F_BF + 1)[c] = by;
-  fld(base, g, F_BF + 2)[c] = bz;
-  if (ix && jy && kz) {
-    const double isg = 1.0 / sqrt(det_gamma(load_met(base, g, c)));
-    fld(base, g, F_BC + 0)[c] = 0.5 * (bx + face_bx(Ay, Az, B0x, g, c + 1)) * isg;
-    fld(base, g, F_BC + 1)[c] = 0.5 * (by + face_by(Ax, Az, B0y, g, c + g.sy)) * isg;
-    fld(base, g, F_BC + 2)[c] = 0.5 * (bz + face_bz(Ax, Ay, B0z, g, c + g.sz)) * isg;
-  }
 }
 
 // G16: static face field B~0^d = mean over the two cells sharing the face of
@@ -287,93 +296,6 @@ __device__ __forceinline__ void cell_speeds(const Prim& P, const Met& M, const E
 #pragma unroll
   for (int d = 0; d < 3; d++)
     if (!(s[d] == s[d])) s[d] = 0.0;  // a NaN never wins the max (same as `s > m`)
-}
-
-// -------------------------------------------------------------------------- con2prim
-// A2 (+A8 when want_speed): interior cells.  Reads D~,S~_j,tau~, B_c, gamma_ij; writes
-// rho,v^i,p and, where a floor/cap acted, the rewritten conserved variables.
-__global__ void __launch_bounds__(128)
-k_con2prim(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
-           DevState* __restrict__ st, int want_speed) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  const bool in = i < g.nx && j < g.ny;
-  double s[3] = {0.0, 0.0, 0.0};
-  int bits = 0, iters = 0;
-  if (in) {
-    const long long c = g.at(i, j, k);
-    const Met M = load_met(base, g, c);
-    const double sg = sqrt(det_gamma(M));
-    const double isg = 1.0 / sg;
-    double U[5], P5[5];
-#pragma unroll
-    for (int r = 0; r < 5; r++) U[r] = fld(base, g, F_Y + r)[c] * isg;  // undensitise, eq. (17)
-    const double Bx = fld(base, g, F_BC + 0)[c], By = fld(base, g, F_BC + 1)[c],
-                 Bz = fld(base, g, F_BC + 2)[c];
-    int rewrite;
-    bits = con2prim(U, Bx, By, Bz, M, E, mask != nullptr && mask[c] != 0, P5, iters, rewrite);
-#pragma unroll
-    for (int r = 0; r < 5; r++) fld(base, g, F_P + r)[c] = P5[r];
-    if (rewrite & 1) fld(base, g, F_Y + 0)[c] = sg * U[0];
-    if (rewrite & 2) {
-#pragma unroll
-      for (int r = 1; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
-    }
-    if (want_speed) {
-      const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
-      cell_speeds(P, M, E, s);
-    }
-  }
-  // counters: integer sums and maxima, order independent
-  const unsigned any = __ballot_sync(0xffffffffu, bits != 0);
-  if (any) {
-    const int nf = __popc(__ballot_sync(0xffffffffu, (bits & 2) != 0));
-    const int np = __popc(__ballot_sync(0xffffffffu, (bits & 4) != 0));
-    const int na = __popc(__ballot_sync(0xffffffffu, (bits & 1) != 0));
-    const int nw = __popc(__ballot_sync(0xffffffffu, (bits & 8) != 0));
-    if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0) {
-      if (nf) atomicAdd((unsigned long long*)&st->c2p_fail, (unsigned long long)nf);
-      if (np) atomicAdd((unsigned long long*)&st->p_fix, (unsigned long long)np);
-      if (na) atomicAdd((unsigned long long*)&st->atmo, (unsigned long long)na);
-      if (nw) atomicAdd((unsigned long long*)&st->w_cap, (unsigned long long)nw);
-    }
-  }
-  int mi = iters;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) mi = max(mi, __shfl_xor_sync(0xffffffffu, mi, o));
-  if (((threadIdx.x + blockDim.x * threadIdx.y) & 31) == 0 && mi > 0)
-    atomicMax((long long*)&st->c2p_maxiter, (long long)mi);
-  if (want_speed) block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
-}
-
-// stand-alone A8 (used after set_prims / set_vecpot)
-__global__ void __launch_bounds__(128)
-k_maxspeed(const double* __restrict__ base, Geom g, Eos E, DevState* __restrict__ st) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  double s[3] = {0.0, 0.0, 0.0};
-  if (i < g.nx && j < g.ny) {
-    const long long c = g.at(i, j, k);
-    cell_speeds(load_prim(base, g, c), load_met(base, g, c), E, s);
-  }
-  block_max3_atomic(s[0], s[1], s[2], st->ms_acc);
-}
-
-// eqs (20)-(22) on the interior: U~ = sqrt(gamma) U(P, B_c)
-__global__ void k_prim2con(double* __restrict__ base, Geom g, Eos E) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  const int j = blockIdx.y * blockDim.y + threadIdx.y;
-  const int k = blockIdx.z;
-  if (i >= g.nx || j >= g.ny) return;
-  const long long c = g.at(i, j, k);
-  const Met M = load_met(base, g, c);
-  const double sg = sqrt(det_gamma(M));
-  double U[5];
-  prim2con(load_prim(base, g, c), M, E, U);
-#pragma unroll
-  for (int r = 0; r < 5; r++) fld(base, g, F_Y + r)[c] = sg * U[r];
 }
 
 // ------------------------------------------------------------ fused post-update kernel

@@ -1,81 +1,9 @@
-// kernels_flux.cuh -- reconstruction + Riemann flux per direction (A3+A4) and the
-// divergence + flux-CT + RK update (A5, A6, A7; the sources of A5 are evaluated in k_post).
+// kernels_flux.cuh -- divergence + flux-CT + RK update (A5, A6, A7; the sources of A5 are
+// evaluated by k_src, kernels_aux.cuh).
 #pragma once
 #include "kernels_aux.cuh"
 
 namespace gk {
-
-// R4: 4-point Lagrange interpolation to the face between cells c-sd and c
-// (adapted per G3)
-__device__ __forceinline__ double lagrange4(const double* __restrict__ q, long long c,
-                                            long long sd) {
-  return (-q[c - 2 * sd] + 9.0 * q[c - sd] + 9.0 * q[c] - q[c + sd]) * 0.0625;
-}
-
-__device__ __forceinline__ Met face_metric(const double* base, const Geom& g, long long c,
-                                           long long sd) {
-  Met M;
-  M.a = lagrange4(fld(base, g, F_MET + 0), c, sd);
-  M.bx = lagrange4(fld(base, g, F_MET + 1), c, sd);
-  M.by = lagrange4(fld(base, g, F_MET + 2), c, sd);
-  M.bz = lagrange4(fld(base, g, F_MET + 3), c, sd);
-  M.gxx = lagrange4(fld(base, g, F_MET + 4), c, sd);
-  M.gxy = lagrange4(fld(base, g, F_MET + 5), c, sd);
-  M.gxz = lagrange4(fld(base, g, F_MET + 6), c, sd);
-  M.gyy = lagrange4(fld(base, g, F_MET + 7), c, sd);
-  M.gyz = lagrange4(fld(base, g, F_MET + 8), c, sd);
-  M.gzz = lagrange4(fld(base, g, F_MET + 9), c, sd);
-  return M;
-}
-
-// ------------------------------------------------------------------------------ fluxes
-// Generic one-thread-per-face kernel (any block shape).  Faces f = 0..n_D along D, transverse
-// cells with the 1-cell apron flux-CT needs (R10).  Face index = index of its upper cell.
-template <int D>
-__global__ void __launch_bounds__(128)
-k_flux_face(double* __restrict__ base, Geom g, Eos E) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x - (D == 0 ? 0 : 1);
-  const int j = blockIdx.y * blockDim.y + threadIdx.y - (D == 1 ? 0 : 1);
-  const int k = blockIdx.z - (D == 2 ? 0 : 1);
-  if (i > g.nx || j > g.ny) return;  // k is in range by construction of the grid
-  const long long c = g.at(i, j, k);
-  const long long sd = D == 0 ? 1 : (D == 1 ? g.sy : g.sz);
-  const Met M = face_metric(base, g, c, sd);
-  const double det = det_gamma(M);
-  const double idet = 1.0 / det;
-  const double sgf = sqrt(det);
-  const double gdd = inv_gamma_dd<D>(M, idet);
-
-  // flattening coefficients of cells f-1 and f from p and v^D (G8c)
-  double fL = 0.0, fR = 0.0;
-  if (E.recon == 1 && E.flatten) {
-    const double* pp = fld(base, g, F_P + 4);
-    const double* vv = fld(base, g, F_P + 1 + D);
-    const double p0 = pp[c - 3 * sd], p1 = pp[c - 2 * sd], p3 = pp[c], p4 = pp[c + sd],
-                 p2 = pp[c - sd], p5 = pp[c + 2 * sd];
-    fL = ppm_flatten(p0, p1, p3, p4, vv[c - 2 * sd], vv[c]);
-    fR = ppm_flatten(p1, p2, p4, p5, vv[c - sd], vv[c + sd]);
-  }
-  double qL[8], qR[8];
-#pragma unroll
-  for (int v = 0; v < 8; v++) {
-    const double* q = v < 5 ? fld(base, g, F_P + v) : fld(base, g, F_BC + (v - 5));
-    double cc[6];
-#pragma unroll
-    for (int s = 0; s < 6; s++) cc[s] = q[c + (s - 3) * sd];
-    recon_pair(E.recon, cc, fL, fR, qL[v], qR[v]);
-  }
-  // G6: the normal field is the single-valued staggered one
-  const double Bn = fld(base, g, F_BF + D)[c] / sgf;
-  qL[5 + D] = Bn; qR[5 + D] = Bn;
-  const Prim PL = {qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6], qL[7]};
-  const Prim PR = {qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6], qR[7]};
-  double out[7];
-  riemann_face<D>(PL, PR, M, sgf, gdd, E, out);
-  const int fid = D == 0 ? F_FX : (D == 1 ? F_FY : F_FZ);
-#pragma unroll
-  for (int r = 0; r < 7; r++) fld(base, g, fid + r)[c] = out[r];
-}
 
 // ------------------------------------------------------------------------------ update
 // RK stage combination (R12 / G15).  mode: 0 first SSP stage (saves Y0), 1 later SSP stage

@@ -49,10 +49,16 @@ enum FieldId {
   F_W = 73,     // 12: upwind-CT face data, 4 per direction d: a_+, a_- (eq. 34) and the upwind
                 //     transverse velocities vbar^{(d+1)%3}, vbar^{(d+2)%3} (eq. 33); F_W + 4 d + r
   F_GV = 85,    // 5 : Lorenz gauge, on vertices: G_A (eq. 31), F_Psi^x,y,z (eq. 32), alpha
-  F_KS = 90,    // 9 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
-  F_END_RK23 = 90,
-  F_END_RK4 = 99
+  F_FM = 90,    // 33: STATIC face metric, 11 per direction d (the ADM variables are held fixed,
+                //     PAPER.md:61, so the 4-point Lagrange values of R4 are formed once, in
+                //     grmhd_set_metric): F_FM + 11 d + {alpha, beta^x, beta^y, beta^z, gamma_xx,
+                //     gamma_xy, gamma_xz, gamma_yy, gamma_yz, gamma_zz, sqrt(gamma)} on the lower
+                //     d-face of the index
+  F_KS = 123,   // 9 : RK4 accumulator k1 + 2 k2 + 2 k3 (only allocated when rk = 4)
+  F_END_RK23 = 123,
+  F_END_RK4 = 132
 };
+constexpr int NFM = 11;  // static face-metric fields per direction
 
 // device-resident scalars of a handle
 struct DevState {

@@ -184,86 +184,4 @@ __device__ __forceinline__ void char_speeds(const Prim& P, const Pt& s, const Me
   lp = aoden * (mid + root) - bd;
 }
 
-// R5 (last part): floors and velocity cap on a reconstructed face state.
-__device__ __forceinline__ void face_floors(Prim& P, const Met& M, const Eos& E) {
-  if (P.rho < E.rho_atm) P.rho = E.rho_atm;
-  if (P.p < E.p_floor) P.p = E.p_floor;
-  double lx, ly, lz;
-  lower(M, P.vx, P.vy, P.vz, lx, ly, lz);
-  const double v2 = lx * P.vx + ly * P.vy + lz * P.vz;
-  if (v2 > E.v2max) {
-    const double f = sqrt(E.v2max / v2);
-    P.vx *= f; P.vy *= f; P.vz *= f;
-  }
-}
-
-// One side of a face: conserved state U[8], coordinate flux G = alpha F^D of eq. (18)
-// (the alpha is reading G10) and the two speeds.
-// Rows: 0 D, 1-3 S_j, 4 tau, 5-7 B^k.
-template <int D>
-__device__ __forceinline__ void side_state(const Prim& P, const Met& M, double gdd,
-                                           const Eos& E, double U[8], double Gf[8], double& lm,
-                                           double& lp) {
-  const Pt s = point_state(P, M, E);
-  const double eW2 = (s.rhoh + s.b2) * s.W * s.W;
-  const double ptot = P.p + 0.5 * s.b2;
-  U[0] = P.rho * s.W;
-  U[1] = eW2 * s.vlx - s.ab0 * s.blx;
-  U[2] = eW2 * s.vly - s.ab0 * s.bly;
-  U[3] = eW2 * s.vlz - s.ab0 * s.blz;
-  U[4] = eW2 - ptot - s.ab0 * s.ab0 - U[0];
-  U[5] = P.Bx; U[6] = P.By; U[7] = P.Bz;
-  const double vtx = M.a * P.vx - M.bx;  // v~^i = alpha v^i - beta^i
-  const double vty = M.a * P.vy - M.by;
-  const double vtz = M.a * P.vz - M.bz;
-  const double vtd = D == 0 ? vtx : (D == 1 ? vty : vtz);
-  const double vd = D == 0 ? P.vx : (D == 1 ? P.vy : P.vz);
-  const double Bd = D == 0 ? P.Bx : (D == 1 ? P.By : P.Bz);
-  const double aBdW = M.a * Bd * s.iW;   // alpha B^d / W
-  const double ap = M.a * ptot;
-  Gf[0] = U[0] * vtd;
-  Gf[1] = U[1] * vtd - s.blx * aBdW + (D == 0 ? ap : 0.0);
-  Gf[2] = U[2] * vtd - s.bly * aBdW + (D == 1 ? ap : 0.0);
-  Gf[3] = U[3] * vtd - s.blz * aBdW + (D == 2 ? ap : 0.0);
-  Gf[4] = U[4] * vtd + ap * vd - s.ab0 * aBdW;
-  Gf[5] = P.Bx * vtd - Bd * vtx;
-  Gf[6] = P.By * vtd - Bd * vty;
-  Gf[7] = P.Bz * vtd - Bd * vtz;
-  char_speeds<D>(P, s, M, gdd, E, lm, lp);
-}
-
-// R7: HLLE eq. (29) PAPER.md:196 or LxF eq. (30) PAPER.md:203 on the face states PL, PR
-// (floors applied here).  Writes sgf * F^ for the rows that are stored: out[0..4] hydro,
-// out[5], out[6] = the two transverse B rows in cyclic order (D+1, D+2)%3.
-template <int D>
-__device__ __forceinline__ void riemann_face(Prim PL, Prim PR, const Met& M, double sgf,
-                                             double gdd, const Eos& E, double out[7]) {
-  face_floors(PL, M, E);
-  face_floors(PR, M, E);
-  double UL[8], UR[8], GL[8], GR[8], lmL, lpL, lmR, lpR;
-  side_state<D>(PL, M, gdd, E, UL, GL, lmL, lpL);
-  side_state<D>(PR, M, gdd, E, UR, GR, lmR, lpR);
-  const double cmax = fmax(0.0, fmax(lpL, lpR));
-  const double cmin = -fmin(0.0, fmin(lmL, lmR));
-  double F[8];
-  if (E.riemann == 1) {
-    const double cw = fmax(cmax, cmin);
-#pragma unroll
-    for (int r = 0; r < 8; r++) F[r] = 0.5 * (GR[r] + GL[r] - cw * (UR[r] - UL[r]));
-  } else if (cmax + cmin < 1e-300) {
-#pragma unroll
-    for (int r = 0; r < 8; r++) F[r] = 0.5 * (GL[r] + GR[r]);
-  } else {
-    const double inv = 1.0 / (cmax + cmin);
-    const double cc = cmax * cmin;
-#pragma unroll
-    for (int r = 0; r < 8; r++)
-      F[r] = (cmin * GR[r] + cmax * GL[r] - cc * (UR[r] - UL[r])) * inv;
-  }
-#pragma unroll
-  for (int r = 0; r < 5; r++) out[r] = sgf * F[r];
-  out[5] = sgf * F[5 + (D + 1) % 3];
-  out[6] = sgf * F[5 + (D + 2) % 3];
-}
-
 }  // namespace gk

@@ -1,179 +1,11 @@
-// recon_c2p.cuh -- reconstruction (R5/G7/G8), con2prim (R14) and source terms (R9/G11).
-// Device-only restatements of PAPER.md:190-192 (reconstruction), PAPER.md:256-295 +
-// PAPER.md:326 (con2prim + atmosphere) and eq. (19) PAPER.md:125 (sources).
+// recon_c2p.cuh -- con2prim (R14) and source terms (R9/G11).
+// Device-only restatements of PAPER.md:256-295 + PAPER.md:326 (con2prim + atmosphere) and
+// eq. (19) PAPER.md:125 (sources).  (The reconstruction lives in flux_face.cuh.)
 #pragma once
 #include "phys.cuh"
+#include "c2p_1d.cuh"
 
 namespace gk {
-
-// ------------------------------------------------------------------------ reconstruction
-// G7: minmod(a,b) = 0 if a*b <= 0 else sign(a) min(|a|,|b|)
-__device__ __forceinline__ double minmod(double a, double b) {
-  if (a * b <= 0.0) return 0.0;
-  const double m = fmin(fabs(a), fabs(b));
-  return a > 0.0 ? m : -m;
-}
-
-// G8(a): monotonised central slope of a cell from its two neighbours.
-__device__ __forceinline__ double ppm_slope(double qm1, double q0, double qp1) {
-  const double dp = qp1 - q0, dm = q0 - qm1;
-  if (dp * dm > 0.0) {
-    const double d = 0.5 * (qp1 - qm1);
-    const double lim = fmin(fabs(d), fmin(2.0 * fabs(dp), 2.0 * fabs(dm)));
-    return d > 0.0 ? lim : -lim;
-  }
-  return 0.0;
-}
-
-// G8(c): flattening coefficient of a cell from p_{i-2..i+2} and v^d_{i-1}, v^d_{i+1}.
-__device__ __forceinline__ double ppm_flatten(double pm2, double pm1, double pp1, double pp2,
-                                              double vm1, double vp1) {
-  const double dp1 = pp1 - pm1;
-  const double dp2 = pp2 - pm2;
-  if (fabs(dp1) > 0.33 * fmin(pp1, pm1) && vm1 > vp1) {
-    if (dp2 == 0.0) return 1.0;
-    const double f = 10.0 * (dp1 / dp2 - 0.75);
-    return fmin(1.0, fmax(0.0, f));
-  }
-  return 0.0;
-}
-
-// G8(b): 4th-order interface value between cells (q0 | q1) from the two limited slopes.
-__device__ __forceinline__ double ppm_iface(double q0, double q1, double dm0, double dm1) {
-  return 0.5 * (q0 + q1) - (dm1 - dm0) * (1.0 / 6.0);
-}
-
-// G8(c,d): flatten + monotonise the parabola of one cell; qm = q^-_i, qp = q^+_i.
-__device__ __forceinline__ void ppm_limit(double q0, double f, double& qm, double& qp) {
-  qp = f * q0 + (1.0 - f) * qp;
-  qm = f * q0 + (1.0 - f) * qm;
-  if ((qp - q0) * (q0 - qm) <= 0.0) {
-    qp = q0; qm = q0;
-  } else {
-    const double Dq = qp - qm;
-    const double m = q0 - 0.5 * (qp + qm);
-    const double D26 = Dq * Dq * (1.0 / 6.0);
-    if (Dq * m > D26) qm = 3.0 * q0 - 2.0 * qp;
-    else if (-D26 > Dq * m) qp = 3.0 * q0 - 2.0 * qm;
-  }
-}
-
-// Face states of one variable from the 6 cells c[0..5] = f-3..f+2 around face f:
-// qL from cell f-1, qR from cell f.  fL/fR are the flattening coefficients of those cells.
-__device__ __forceinline__ void recon_pair(int recon, const double c[6], double fL, double fR,
-                                           double& qL, double& qR) {
-  if (recon == 0) {
-    qL = c[2] + 0.5 * minmod(c[2] - c[1], c[3] - c[2]);
-    qR = c[3] - 0.5 * minmod(c[3] - c[2], c[4] - c[3]);
-  } else {
-    const double d1 = ppm_slope(c[0], c[1], c[2]);
-    const double d2 = ppm_slope(c[1], c[2], c[3]);
-    const double d3 = ppm_slope(c[2], c[3], c[4]);
-    const double d4 = ppm_slope(c[3], c[4], c[5]);
-    const double i12 = ppm_iface(c[1], c[2], d1, d2);  // interface f-3/2
-    const double i23 = ppm_iface(c[2], c[3], d2, d3);  // interface f-1/2 (this face)
-    const double i34 = ppm_iface(c[3], c[4], d3, d4);  // interface f+1/2
-    double qm = i12, qp = i23;
-    ppm_limit(c[2], fL, qm, qp);
-    qL = qp;
-    qm = i23; qp = i34;
-    ppm_limit(c[3], fR, qm, qp);
-    qR = qm;
-  }
-}
-
-// --------------------------------------------------------- con2prim, 1-D backup scheme
-// Row F4: the scheme of PAPER.md:297-320 (eqs 42-45) the paper falls back to when the 2-D
-// Newton iteration fails.  One unknown x = h W, bracketed by
-// max(1 + q - s, 1) < x < 2 + 2q - s, root of eq. (43) by Brent's method.  Readings G23-G25 of
-// DESIGN.md (t^2/x^2 in eq. (45); 1/W^2 kept in [1/w_max^2, 1]; eps^ >= 0 while iterating).
-// Rare path: plain IEEE division and square root, not inlined.
-struct C2p1d {
-  double q, r, s, t, Gamma, iw2min;
-  __device__ void state(double x, double& W, double& eps) const {
-    double iw2 = 1.0 - (r * x * x + t * t * (2.0 * x + s)) / (x * x * (x + s) * (x + s));  // (44)
-    iw2 = fmin(fmax(iw2, iw2min), 1.0);
-    W = 1.0 / sqrt(iw2);
-    eps = -1.0 + x / W * (1.0 - W * W) +
-          W * (1.0 + q - s + 0.5 * (t * t / (x * x) + s * iw2));  // (45)
-    eps = fmax(eps, 0.0);
-  }
-  __device__ double f(double x) const {  // (43), h^ = 1 + Gamma eps^ for the ideal fluid
-    double W, eps;
-    state(x, W, eps);
-    return x - (1.0 + Gamma * eps) * W;
-  }
-};
-
-// U = undensitised (D, S_j, tau).  Returns true and rho, v^i, eps on success.
-__device__ __noinline__ bool con2prim_1d(const double* U, double Bx, double By, double Bz,
-                                         const Met& M, const Eos& E, double& rho, double& vx,
-                                         double& vy, double& vz, double& eps, int& iters) {
-  const double D = U[0], Sx = U[1], Sy = U[2], Sz = U[3], tau = U[4];
-  const double idet = 1.0 / det_gamma(M);
-  const Sym3 gu = inv_gamma(M, idet);
-  const double Sux = gu.xx * Sx + gu.xy * Sy + gu.xz * Sz;
-  const double Suy = gu.xy * Sx + gu.yy * Sy + gu.yz * Sz;
-  const double Suz = gu.xz * Sx + gu.yz * Sy + gu.zz * Sz;
-  const double S2 = Sux * Sx + Suy * Sy + Suz * Sz;
-  double Blx, Bly, Blz;
-  lower(M, Bx, By, Bz, Blx, Bly, Blz);
-  const double B2 = Blx * Bx + Bly * By + Blz * Bz;
-  const double BS = Bx * Sx + By * Sy + Bz * Sz;
-  C2p1d c;  // eq. (42)
-  c.Gamma = E.Gamma; c.iw2min = 1.0 - E.v2max;
-  c.q = tau / D; c.r = S2 / (D * D); c.s = B2 / D; c.t = BS / (D * sqrt(D));
-  double a = fmax(1.0 + c.q - c.s, 1.0), b = 2.0 + 2.0 * c.q - c.s;
-  iters = 0;
-  if (!(b > a)) return false;
-  // Brent: bracket [b, cc] with |f(b)| <= |f(cc)|, a = previous iterate
-  double fa = c.f(a), fb = c.f(b);
-  bool found = false;
-  double x = 0.0;
-  if (fa == 0.0) { x = a; found = true; }
-  else if (fb == 0.0) { x = b; found = true; }
-  else if (!(fa * fb < 0.0)) return false;
-  double cc = a, fc = fa, d = b - a, e = d;
-  for (int it = 1; it <= 100 && !found; it++) {
-    iters = it;
-    if ((fb > 0.0) == (fc > 0.0)) { cc = a; fc = fa; d = b - a; e = d; }
-    if (fabs(fc) < fabs(fb)) { a = b; b = cc; cc = a; fa = fb; fb = fc; fc = fa; }
-    const double tol1 = 2.0 * 2.220446049250313e-16 * fabs(b) + 0.5 * 1e-14 * fabs(b);
-    const double xm = 0.5 * (cc - b);
-    if (fabs(xm) <= tol1 || fb == 0.0) { x = b; found = true; break; }
-    if (fabs(e) >= tol1 && fabs(fa) > fabs(fb)) {
-      const double sv = fb / fa;
-      double pp, qq;
-      if (a == cc) {
-        pp = 2.0 * xm * sv;
-        qq = 1.0 - sv;
-      } else {
-        const double qa = fa / fc, rr = fb / fc;
-        pp = sv * (2.0 * xm * qa * (qa - rr) - (b - a) * (rr - 1.0));
-        qq = (qa - 1.0) * (rr - 1.0) * (sv - 1.0);
-      }
-      if (pp > 0.0) qq = -qq;
-      pp = fabs(pp);
-      if (2.0 * pp < fmin(3.0 * xm * qq - fabs(tol1 * qq), fabs(e * qq))) { e = d; d = pp / qq; }
-      else { d = xm; e = d; }
-    } else {
-      d = xm; e = d;
-    }
-    a = b; fa = fb;
-    b += fabs(d) > tol1 ? d : (xm > 0.0 ? tol1 : -tol1);
-    fb = c.f(b);
-  }
-  if (!found || !isfinite(x)) return false;
-  double W;
-  c.state(x, W, eps);
-  rho = D / W;
-  const double z = D * x;  // (vii): z = rho W x
-  const double izB = 1.0 / (z + B2), BSz = BS / z;
-  vx = (Sux + BSz * Bx) * izB;  // eq. (41c)
-  vy = (Suy + BSz * By) * izB;
-  vz = (Suz + BSz * Bz) * izB;
-  return isfinite(rho) && isfinite(eps) && isfinite(vx) && isfinite(vy) && isfinite(vz);
-}
 
 // ---------------------------------------------------------------------------- con2prim
 // R14: Noble 2-D Newton-Raphson on (z, v^2), eqs (36)-(41) PAPER.md:260-295; atmosphere

@@ -168,9 +168,9 @@ def test_backup_con2prim_in_the_step():
 def test_upwind_ct_matches_oracle():
     """Row F1: E on the edges by the upwind constrained transport (eqs 33-35) on both sides;
     wide blocks (TMA kernels with the 3-cell apron), a narrow one (lanes-along-D kernel in every
-    direction), minmod, RK4, and the x fluxes through the TMA kernel."""
+    direction), minmod, RK4, and the lanes-along-D kernel on a wide block."""
     cases = [(wl.kerr_blob(40), None), (wl.blast(44), None), (wl.c2p_stress(36), None),
-             (wl.bns_like(32), None), (wl.kerr_blob(40), {"flux_x_rows": 0.0}),
+             (wl.bns_like(32), None), (wl.kerr_blob(40), {"flux_kernel": 0.0}),
              (wl.kerr_blob(40), {"uct_passes": 0.0}),   # the per-edge kernel k_emf_uct
              (wl.alfven_wave(16, 1, 1, axis=0), None), (wl.balsara1(64, 4, 4), None),
              (wl.make(1), None)]          # 128^3: several groups, segments and waves
@@ -279,15 +279,15 @@ def test_odd_and_non_cubic_blocks():
     of the TMA kernel and the 27-face segments of the lanes-along-D kernel."""
     w = wl.kerr_blob(72)
     for (nx, ny, nz) in ((37, 33, 35), (65, 31, 34), (28, 55, 63)):
-        for opts in (None, {"flux_x_rows": 0.0}):
+        for opts in (None, {"flux_kernel": 0.0}):
             _one_step_case(_crop(w, nx, ny, nz, f"kerr_crop_{nx}x{ny}x{nz}"), gpu_options=opts)
     _one_step_case(wl.c2p_stress(45))     # periodic, odd
 
 
 def test_every_flux_kernel_is_covered():
-    """The three implementations of A3+A4 give the oracle's result: k_flux_xrow + k_flux_tma
-    (default), k_flux_tma for x as well, and the marching kernel k_flux_march everywhere."""
-    for opts in ({"flux_x_rows": 0.0}, {"flux_kernel": 0.0}):
+    """Both implementations of A3+A4 give the oracle's result: k_flux_xrow for x + k_flux_tma for
+    y and z (default, every other test), and k_flux_xrow in all three directions."""
+    for opts in ({"flux_kernel": 0.0},):
         _one_step_case(wl.kerr_blob(40), gpu_options=opts)
         _one_step_case(wl.blast(44), gpu_options=opts)
         w = wl.c2p_stress(36)
@@ -395,9 +395,9 @@ def test_cuda_graph_step_is_bit_identical_to_eager():
             assert np.array_equal(x, y), w.name
         sa, sb = a.stats(), b.stats()
         assert sa["steps"] == sb["steps"] == 6 and sa["t"] == sb["t"] and sa["dt"] == sb["dt"]
-        # change the launch sequence after the capture: other x-flux kernel on both
-        a.set_option("flux_x_rows", 0)
-        b.set_option("flux_x_rows", 0)
+        # change the launch sequence after the capture: other y/z-flux kernel on both
+        a.set_option("flux_kernel", 0)
+        b.set_option("flux_kernel", 0)
         a.step(4, w.cfl)
         b.step(4, w.cfl)
         for x, y in zip(to_np(a.get_cons()), to_np(b.get_cons())):

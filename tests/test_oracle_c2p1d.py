@@ -123,3 +123,60 @@ def test_backup_takes_over_when_the_2d_scheme_fails():
         else:
             assert bb == bits
     assert nback > 50
+
+
+def _numpy_cons(P, M, Gamma):
+    """Eqs (13), (37), (20)-(22) written out in numpy; does not call
+    the oracle."""
+    g = gam_mat(M)
+    rho, v, p, B = P[0], P[1:4], P[4], P[5:8]
+    vl, Bl = g @ v, g @ B
+    W = 1.0 / np.sqrt(1.0 - v @ vl)
+    ab0 = W * (B @ vl)                               # alpha b^0, eq. (13)
+    b2 = (B @ Bl + ab0 ** 2) / W ** 2                # b^2, eq. (13)
+    bl = Bl / W + ab0 * vl                           # b_i, eq. (37)
+    h = 1.0 + Gamma * p / ((Gamma - 1.0) * rho)      # eq. (46)
+    D = rho * W                                      # eq. (20)
+    S = (rho * h + b2) * W ** 2 * vl - ab0 * bl      # eq. (21)
+    tau = (rho * h + b2) * W ** 2 - (p + 0.5 * b2) - ab0 ** 2 - D   # eq. (22)
+    return D, S, tau, W, h
+
+
+def test_P15_recovered_state_satisfies_eqs_20_22_and_43_45_in_numpy():
+    """The pin that does not pass through the oracle's own eq. (44)/(45) code: conserved
+    states that come from NO known primitive state (a consistent state with tau and S_j pushed
+    away from it) are recovered by the 1-D scheme; the recovered primitives, put through eqs
+    (20)-(22) in numpy, must give back the conserved input, and x = hW of the recovered state
+    must satisfy eqs (44), (45), (43) evaluated in numpy with the q, r, s, t of eq. (42)."""
+    prim, met = wl.c2p_states(600)
+    o = _opts()
+    rng = np.random.default_rng(4245)
+    worst = np.zeros(5)
+    for n in range(prim.shape[1]):
+        P, M = prim[:, n], met[:, n]
+        U = ref.prim2con_pt(P, M, G53)
+        U[4] *= 1.0 + 0.2 * rng.random()             # more energy: stays inside the physical region
+        U[1:4] *= 1.0 - 0.1 * rng.random()           # less momentum
+        p1, st, _ = ref.con2prim1d_pt(U, M, o)
+        assert st == 0, n
+        Prec = np.concatenate([p1, U[5:8]])
+        D, S, tau, W, h = _numpy_cons(Prec, M, G53)
+        sc = max(np.abs(U[1:4]).max(), U[4] + U[0])
+        worst[0] = max(worst[0], abs(D - U[0]) / U[0])
+        worst[1] = max(worst[1], np.abs(S - U[1:4]).max() / sc)
+        worst[2] = max(worst[2], abs(tau - U[4]) / (U[4] + U[0]))
+        # eqs (42)-(45) in numpy at x = hW of the recovered state
+        g = gam_mat(M)
+        gu = np.linalg.inv(g)
+        B = U[5:8]
+        q, r = U[4] / U[0], (U[1:4] @ gu @ U[1:4]) / U[0] ** 2
+        s, t = (B @ g @ B) / U[0], (B @ U[1:4]) / U[0] ** 1.5
+        x = h * W
+        iw2 = 1.0 - (r * x * x + t * t * (2.0 * x + s)) / (x * x * (x + s) ** 2)      # (44)
+        eps = -1.0 + x * np.sqrt(iw2) * (1.0 - 1.0 / iw2) + \
+            (1.0 + q - s + 0.5 * (t * t / (x * x) + s * iw2)) / np.sqrt(iw2)          # (45), G23
+        worst[3] = max(worst[3], abs(iw2 - 1.0 / W ** 2) * W ** 2)
+        worst[4] = max(worst[4], abs(x - (1.0 + G53 * eps) / np.sqrt(iw2)) / x)       # (43)
+        assert 1.0 + q - s < x < 2.0 + 2.0 * q - s
+    assert worst[0] < 1e-11 and worst[1] < 1e-10 and worst[2] < 1e-10, worst
+    assert worst[3] < 1e-9 and worst[4] < 1e-9, worst
