@@ -56,12 +56,37 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def traffic_for(workload_name):
-    """dram bytes per flux launch from the committed ncu capture, if one exists for this workload."""
+def kernel_source_hash():
+    """sha256 over the CUDA sources the library was built from (sorted by name): ties a committed
+    ncu capture to the kernels this run executes (the GPU box has no .git to ask)."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2406_11669_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def traffic_for(workload_name, options):
+    """DRAM bytes per flux launch (dram__bytes_read.sum + dram__bytes_write.sum of one
+    `ncu --set full` capture, profiles/traffic.json) -- only if that capture was taken on THESE
+    kernel sources, this workload and these options; otherwise null: a stale number is not
+    printed beside live ones."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(p):
-        return json.load(open(p)).get(workload_name)
-    return None
+    if not os.path.exists(p):
+        return None, {"traffic_source": None}
+    t = json.load(open(p))
+    meta = {"traffic_source": t.get("_source"), "traffic_source_commit": t.get("_commit"),
+            "traffic_source_kernel_hash": t.get("_kernel_hash")}
+    same = (t.get("_kernel_hash") == kernel_source_hash() and not options
+            and workload_name in t)
+    if not same:
+        meta["traffic_note"] = "capture does not match this run (kernel sources, workload or options): not reported"
+        return None, meta
+    meta["fp64_pipe_active_pct_ncu"] = t.get("_fp64_pipe_active_pct")
+    return t[workload_name], meta
 
 
 class ClockSampler:
@@ -139,14 +164,20 @@ def sample_workload(args):
     return wl.make(args.config, n), f"same generator at {n}^3"
 
 
-def cpu_baseline(args, target_s=12.0):
+def cpu_baseline(args, target_s=10.0, target_1core_s=8.0):
+    """The oracle as it stands on all host cores and, beside it, on ONE core."""
     ws, what = sample_workload(args)
     cores = os.cpu_count() or 1
     v1, t1 = oracle_throughput(ws, 1, cores)
     steps = int(max(1, min(200, target_s / max(t1, 1e-3))))
     v, t = oracle_throughput(ws, steps, cores)
+    _, s1 = oracle_throughput(ws, 1, 1)
+    steps1 = int(max(1, min(50, target_1core_s / max(s1, 1e-3))))
+    vs, ts = oracle_throughput(ws, steps1, 1)
     return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{what}, {steps} RK{ws.stages} steps, {t:.1f} s wall, OpenMP {cores} threads"}
+            "sample": f"{what}, {steps} RK{ws.stages} steps, {t:.1f} s wall, OpenMP {cores} threads",
+            "one_core": {"value": vs, "unit": UNIT, "cores": 1,
+                         "sample": f"{what}, {steps1} RK{ws.stages} steps, {ts:.1f} s wall"}}
 
 
 def run_reference(args):
@@ -361,22 +392,26 @@ def run_b200(args):
     flux_n = sum(kt[k][1] for k in ("flux_x", "flux_y", "flux_z")) or 1
     flux_avg = flux_ms / flux_n
     achieved = FLUX_BYTES_PER_CELL_DIR * w.ncells / (flux_avg * 1e-3) / 1e9
+    traffic, traffic_meta = traffic_for(w.name, options)
     roofline = {"kernel": "flux (reconstruct + Riemann, average of x/y/z launches)",
                 "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic_for(w.name),
-                "fp64_pipe_active_pct_ncu": traffic_for("_fp64_pipe_active_pct"),
+                "frac": achieved / peak, "traffic": traffic,
                 "alg_bytes_per_launch": FLUX_BYTES_PER_CELL_DIR * w.ncells,
+                "alg_bytes_note": "208 B per cell-direction = the method's own bytes (SURVEY 8(d): "
+                                  "19 doubles read, 7 written); the kernel reads one more double, "
+                                  "the precomputed sqrt(gamma) of the face (216 B)",
                 "ms_per_launch": flux_avg, "share_of_step": flux_ms / tot_k,
                 "peak_source": peak_src,
                 "step_decomposed_frac": (1400.0 * zone_sub / (ms * 1e-3) / 1e9) / peak,
                 "step_floor_frac": (344.0 * zone_sub / (ms * 1e-3) / 1e9) / peak}
+    roofline.update(traffic_meta)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": w.name, "cells": [w.nx, w.ny, w.nz], "ghosts": 3,
                        "stages_per_step": w.stages, "recon": "ppm" if w.opts["recon"] else "minmod",
-                       "riemann": "hlle", "cfl": w.cfl, "parallelism": "replicas" if world > 1 else "1gpu",
+                       "riemann": "lxf" if w.opts.get("riemann") else "hlle", "cfl": w.cfl, "parallelism": "replicas" if world > 1 else "1gpu",
                        "l2": "inputs larger than L2 (every kernel streams > 126 MB)"
                              if w.ncells >= 128 ** 3 else "working set fits L2 (latency-bound config)",
                        "us_per_substep": 1e3 * ms / (args.steps * w.stages)},

@@ -18,6 +18,10 @@
  *   - Every pointer argument marked [dev|host] may be a CUDA device pointer or a host
  *     pointer (pinned host memory recommended); the library copies with
  *     cudaMemcpyDefault (unified virtual addressing decides the direction).
+ *     INPUT arrays in host memory have been consumed when the set_* call returns (the call
+ *     waits for its copies: the caller may reuse or free them at once); with device sources
+ *     set_* only enqueues on the handle's stream and the arrays must stay unchanged until that
+ *     work has run.  OUTPUT calls (get_*) synchronise the stream before returning.
  *   - The caller owns every buffer, including the workspace (device memory, e.g. a
  *     torch tensor).  The library never allocates device memory for fields; it carves its
  *     structure-of-arrays state out of the workspace.  The workspace must stay alive and
@@ -100,7 +104,12 @@ int grmhd_destroy(grmhd* h);
 
 /* 16 cell-centred padded arrays [dev|host], ghosts SUPPLIED BY THE CALLER, in the order
  * alpha, betax, betay, betaz, gxx, gxy, gxz, gyy, gyz, gzz, kxx, kxy, kxz, kyy, kyz, kzz
- * (ADM variables).  field: host array of 16 pointers. */
+ * (ADM variables).  field: host array of 16 pointers.
+ * The metric is held fixed from this call on: the face values the Riemann solver needs (4-point
+ * Lagrange interpolation along the face normal, and sqrt(gamma) of the face) are
+ * formed here, once.  May be called again on a live handle: the conserved variables, the
+ * cell-centred B, the sources and the max speed are then rebuilt from the current primitives
+ * with the new metric by the next call that needs them. */
 int grmhd_set_metric(grmhd* h, const double* const field[16]);
 
 /* 8 cell-centred padded arrays [dev|host]: rho, vx, vy, vz (Eulerian v^i), press,

@@ -131,6 +131,27 @@ def _ptrs(arrs, n, keep):
     return out
 
 
+def _out_ptrs(arrs, n, shape):
+    """Pointers of OUTPUT buffers: the library writes straight into them, so a buffer that would
+    need a converted copy (wrong dtype, not contiguous, wrong shape) is an error, not a silent
+    write into a temporary."""
+    assert len(arrs) == n, f"expected {n} fields"
+    out = (C.c_void_p * n)()
+    for i, a in enumerate(arrs):
+        if isinstance(a, np.ndarray):
+            ok = a.dtype == np.float64 and a.flags["C_CONTIGUOUS"] and a.flags["WRITEABLE"]
+            ptr = a.ctypes.data
+        elif isinstance(a, torch.Tensor):
+            ok = a.dtype == torch.float64 and a.is_contiguous()
+            ptr = a.data_ptr()
+        else:
+            raise TypeError("output fields must be torch tensors or numpy arrays")
+        if not ok or tuple(a.shape) != tuple(shape):
+            raise ValueError(f"output field {i}: need a contiguous fp64 buffer of shape {tuple(shape)}")
+        out[i] = ptr
+    return out
+
+
 class Solver:
     """One handle of the C ABI.  Inputs: torch tensors (CUDA or pinned/pageable host) or
     numpy arrays, fp64, shapes (nz+6, ny+6, nx+6) / staggered (nz+7, ny+7, nx+7)."""
@@ -227,8 +248,7 @@ class Solver:
             else:
                 out = [torch.empty(shape, dtype=torch.float64, device=self.device)
                        for _ in range(n)]
-        keep = []
-        self._chk(fn(self.h, _ptrs(out, n, keep)), what)
+        self._chk(fn(self.h, _out_ptrs(out, n, shape)), what)
         return out
 
     def get_prims(self, out=None, host=False):

@@ -40,6 +40,7 @@ struct grmhd {
   bool tma_ok = false;
   int uct_nseg = 16;     // segments of the marching passes along y and z
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
+  int nsm = 148;         // multiprocessors of the device (queried at create)
   int flux_impl = 1;     // 1: y and z fluxes by k_flux_tma (blocks at least 32 cells wide in x),
                          // 0: k_flux_xrow (lanes along the flux direction) everywhere
   // CUDA graph of one RK step (launch-bound small blocks): the first step after a change of
@@ -333,7 +334,7 @@ int after_stage(grmhd* h, bool want_speed) {
 int apron_width(const grmhd* h) { return h->E.emf ? 3 : 1; }  // G27: PPM face -> edge stencils
 
 template <int D, int RECON>
-int launch_flux_xrow(grmhd* h, int mode) {
+int launch_flux_xrow(grmhd* h, int mode, cudaStream_t st) {
   const Geom& g = h->g;
   const int ap = apron_width(h);
   const int nsd = (g.n(D) + 1 + FX_VALID - 1) / FX_VALID;
@@ -342,11 +343,11 @@ int launch_flux_xrow(grmhd* h, int mode) {
   const long long nitems = npen * nsd;
   const long long nblk = (nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
   if (h->E.emf)
-    k_flux_xrow<D, RECON, true><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd,
-                                                                        nitems, ap, mode);
+    k_flux_xrow<D, RECON, true><<<(unsigned)nblk, FX_THREADS, 0, st>>>(h->base, g, h->E, nsd,
+                                                                      nitems, ap, mode);
   else
-    k_flux_xrow<D, RECON, false><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd,
-                                                                         nitems, ap, mode);
+    k_flux_xrow<D, RECON, false><<<(unsigned)nblk, FX_THREADS, 0, st>>>(h->base, g, h->E, nsd,
+                                                                       nitems, ap, mode);
   h->launches++;
   return GRMHD_OK;
 }
@@ -425,7 +426,10 @@ int launch_flux_tma_v(grmhd* h) {
   h->launches++;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return cuda_fail(h, e, "k_flux_tma");
-  return launch_flux_xrow<D, RECON>(h, 1);  // the apron columns along x
+  // the 2 ap apron columns along x.  (Run beside the main kernel on a second stream they cost
+  // MORE, measured 0.93 against 0.89 ms: their blocks take register space the main kernel's
+  // third block per SM needs.)
+  return launch_flux_xrow<D, RECON>(h, 1, h->s);
 }
 
 template <int D, int RECON>
@@ -438,7 +442,7 @@ int launch_flux_dr(grmhd* h) {
   if (D != 0 && h->flux_impl == 1 && h->tma_ok && h->g.nx >= 32) {
     if constexpr (D != 0) return launch_flux_tma<D, RECON>(h);
   }
-  return launch_flux_xrow<D, RECON>(h, 0);
+  return launch_flux_xrow<D, RECON>(h, 0, h->s);
 }
 
 template <int D>
@@ -645,6 +649,14 @@ int grmhd_create(int nx, int ny, int nz, int ghosts, const double dx[3], const g
     return GRMHD_ECUDA;
   }
   h->tma_ok = make_tensor_maps(h);
+  {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
+      h->nsm = nsm;
+    else
+      cudaGetLastError();
+  }
   *out = h;
   return GRMHD_OK;
 }

@@ -19,19 +19,13 @@ TOL1 = 1e-11
 TOL100 = 1e-9
 
 
-REPORT = []
+from tests.conftest import PARITY_REPORT as REPORT   # written out by --parity-report PATH
 
-
-@pytest.fixture(scope="module", autouse=True)
-def _dump_report():
-    """Write the measured parity errors where the GPU run leaves its artefacts."""
-    yield
-    import json
-    import os
-    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
-    os.makedirs(out, exist_ok=True)
-    with open(os.path.join(out, "parity_errors.json"), "w") as f:
-        json.dump(REPORT, f, indent=1)
+# Bounds that are NOT north_star numbers: after a SECOND step on data with
+# switches (pressure fixes, flattening) the oracle's own answer moves by 3e-12 ... 6e-11 when its
+# inputs are perturbed by one ulp (tests/test_oracle_sensitivity.py), so a second step is checked
+# against a bound that only catches a divergence, not rounding.
+TOL_2STEPS = 1e-10
 
 
 def _assert_cons(Ug, Ur, tol, what):
@@ -165,10 +159,17 @@ def test_backup_con2prim_in_the_step():
     g.close()
 
 
+def _A_err(g, r):
+    Ag, Ar = to_np(g.get_vecpot()), r.get_vecpot()
+    amax = max(max(np.abs(a).max() for a in Ar), 1e-300)
+    return max(float(np.abs(Ag[d] - Ar[d]).max() / amax) for d in range(3))
+
+
 def test_upwind_ct_matches_oracle():
     """Row F1: E on the edges by the upwind constrained transport (eqs 33-35) on both sides;
     wide blocks (TMA kernels with the 3-cell apron), a narrow one (lanes-along-D kernel in every
-    direction), minmod, RK4, and the lanes-along-D kernel on a wide block."""
+    direction), minmod, RK4, and the lanes-along-D kernel on a wide block.  north_star's bar:
+    1e-11 after ONE step; a second step is checked against TOL_2STEPS."""
     cases = [(wl.kerr_blob(40), None), (wl.blast(44), None), (wl.c2p_stress(36), None),
              (wl.bns_like(32), None), (wl.kerr_blob(40), {"flux_kernel": 0.0}),
              (wl.kerr_blob(40), {"uct_passes": 0.0}),   # the per-edge kernel k_emf_uct
@@ -180,38 +181,40 @@ def test_upwind_ct_matches_oracle():
         g.set_option("emf", 1.0)
         for key, val in (extra or {}).items():
             g.set_option(key, val)
-        nsteps = 1 if "c2p_stress" in w.name else 2   # the stress field is at the edge of the
-        r.step(nsteps, w.cfl)                         # recovery's domain after one step
-        g.step(nsteps, w.cfl)
-        _assert_cons(to_np(g.get_cons()), r.get_cons(), 10 * TOL1, w.name + " uct")
-        Ag, Ar = to_np(g.get_vecpot()), r.get_vecpot()
-        amax = max(max(np.abs(a).max() for a in Ar), 1e-300)
-        for d in range(3):
-            assert np.abs(Ag[d] - Ar[d]).max() / amax <= 10 * TOL1, (w.name, "A", d)
+        r.step(1, w.cfl)
+        g.step(1, w.cfl)
+        _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL1, w.name + " uct, 1 step")
+        assert _A_err(g, r) <= TOL1, w.name
+        if "c2p_stress" not in w.name:    # the stress field leaves the recovery's domain
+            r.step(1, w.cfl)
+            g.step(1, w.cfl)
+            _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL_2STEPS, w.name + " uct, 2 steps")
+            assert _A_err(g, r) <= TOL_2STEPS, w.name
         g.close()
 
 
 def test_lorenz_gauge_matches_oracle():
     """Row F3: generalised Lorenz gauge (eqs 31-32) on both sides, with flux-CT and with the
-    upwind CT: same A_i, same Psi_mhd, same conserved variables; and B is the algebraic-gauge B."""
+    upwind CT: same A_i, same Psi_mhd, same conserved variables after one step (1e-11; a second
+    step against TOL_2STEPS); and B is the algebraic-gauge B."""
     for w, emf in ((wl.kerr_blob(40), 0.0), (wl.bns_like(32), 0.0), (wl.bns_like(32), 1.0),
                    (wl.c2p_stress(36), 0.0)):
         r, g, g0 = make_ref(w), make_gpu(w), make_gpu(w)
-        for s in (r, g):
-            s.set_option("gauge", 1.0)
-            s.set_option("emf", emf)
+        for s_ in (r, g):
+            s_.set_option("gauge", 1.0)
+            s_.set_option("emf", emf)
         g0.set_option("emf", emf)
         nsteps = 1 if "c2p_stress" in w.name else 2
-        for s in (r, g, g0):
-            s.step(nsteps, w.cfl)
-        _assert_cons(to_np(g.get_cons()), r.get_cons(), 10 * TOL1, w.name + " lorenz")
-        Ag, Ar = to_np(g.get_vecpot()), r.get_vecpot()
-        amax = max(max(np.abs(a).max() for a in Ar), 1e-300)
-        for d in range(3):
-            assert np.abs(Ag[d] - Ar[d]).max() / amax <= 10 * TOL1, (w.name, "A", d)
-        Pg, Pr = g.get_psi().cpu().numpy(), r.get_psi()
-        pmax = max(np.abs(Pr).max(), 1e-300)
-        assert np.abs(Pg - Pr)[3:-3, 3:-3, 3:-3].max() / pmax <= 10 * TOL1, w.name
+        for step in range(nsteps):
+            tol = TOL1 if step == 0 else TOL_2STEPS
+            for s_ in (r, g, g0):
+                s_.step(1, w.cfl)
+            _assert_cons(to_np(g.get_cons()), r.get_cons(), tol, f"{w.name} lorenz emf={emf:.0f}, "
+                         f"{step + 1} step")
+            assert _A_err(g, r) <= tol, w.name
+            Pg, Pr = g.get_psi().cpu().numpy(), r.get_psi()
+            pmax = max(np.abs(Pr).max(), 1e-300)
+            assert np.abs(Pg - Pr)[3:-3, 3:-3, 3:-3].max() / pmax <= tol, w.name
         if w.vecpot is not None:
             assert pmax > 0
         # gauge independence of what the hydro path sees
@@ -305,26 +308,56 @@ def test_config3_kerr_full_size_one_step():
     _one_step_case(wl.make(2))            # 256^3 Kerr-Schild: the bench workload
 
 
+def _lorentz_factor(P, metric):
+    """W of the oracle's primitives on the interior (numpy; classifies cells, no parity value)."""
+    g = [m[interior_sl] for m in metric[4:10]]
+    v = [P[1][interior_sl], P[2][interior_sl], P[3][interior_sl]]
+    v2 = (g[0] * v[0] ** 2 + g[3] * v[1] ** 2 + g[5] * v[2] ** 2 +
+          2.0 * (g[1] * v[0] * v[1] + g[2] * v[0] * v[2] + g[4] * v[1] * v[2]))
+    return 1.0 / np.sqrt(np.maximum(1.0 - v2, 1e-300))
+
+
+interior_sl = (slice(3, -3),) * 3
+W_EDGE = 9.5   # config 4 draws W in [1, 10]: cells the step leaves above this are at (or beyond)
+               # the edge of the workload's envelope and of the recovery's well-conditioned range
+
+
 def test_config4_c2p_stress_full_size_one_step():
-    """256^3 generic metric, W up to 10, sigma up to 10.  One RK3 step of this stress field
-    drives a handful of cells to the edge of the con2prim domain (measured: 1 cell of 16.8 M,
-    p/rho = 10, W = 10 after the step), where the recovery amplifies rounding differences of
-    the two fp64 implementations by ~1e5.  So: 1e-11 on every field once
-    at most 1e-6 of the cells are set aside, and 1e-10 on all cells."""
+    """256^3 generic metric, W up to 10, sigma up to 10: north_star's 1e-11 after one step.
+
+    Stated plainly: THE BAR IS NOT MET ON CONFIG 4 AT FULL SIZE -- measured, one cell of 16.8 M
+    (W = 9.89, p/rho = 10.5 after the step) differs by 1.4e-11 in the D norm; every other cell of
+    every field is below 5.1e-12.  The oracle itself moves by 2.3e-11 (64^3) under a one-ulp
+    change of its inputs on this workload (tests/test_oracle_sensitivity.py), in exactly such
+    cells, so 1e-11 is below the noise floor of the reference there.  The test therefore asserts
+    1e-11 on every cell whose oracle Lorentz factor after the step is <= W_EDGE, lists the cells
+    above 1e-11 in the report, requires them all to be edge cells (W > W_EDGE), and bounds those
+    by 1e-10.  Failure counters must agree exactly."""
     w = wl.make(3)
     r, g = make_ref(w), make_gpu(w)
     r.step(1, w.cfl)
     g.step(1, w.cfl)
     Ug, Ur = to_np(g.get_cons()), r.get_cons()
-    _assert_cons(Ug, Ur, 1e-10, w.name + " all cells")
-    ncell = w.nx * w.ny * w.nz
+    W = _lorentz_factor(r.get_prims(), w.metric)
+    edge = W > W_EDGE
+    worst_in, worst_edge, offenders = 0.0, 0.0, []
     for grp in ((0,), (1, 2, 3), (4,), (5, 6, 7)):
         scale = max(np.abs(interior(Ur[q])).max() for q in grp)
         for q in grp:
-            nbad = int((np.abs(interior(Ug[q]) - interior(Ur[q])) > TOL1 * scale).sum())
-            REPORT.append({"case": f"{w.name} field {q}: cells above 1e-11", "tol": 1e-6 * ncell,
-                           "max": nbad})
-            assert nbad <= 1e-6 * ncell, (q, nbad)
+            e = np.abs(interior(Ug[q]) - interior(Ur[q])) / scale
+            worst_in = max(worst_in, float(e[~edge].max()))
+            worst_edge = max(worst_edge, float(e[edge].max()) if edge.any() else 0.0)
+            for k, j, i in np.argwhere(e > TOL1):
+                offenders.append({"field": q, "cell": [int(i), int(j), int(k)], "err": float(e[k, j, i]),
+                                  "W": float(W[k, j, i])})
+    REPORT.append({"case": w.name + " cells with W <= %.1f" % W_EDGE, "tol": TOL1, "max": worst_in})
+    REPORT.append({"case": w.name + " edge cells (W > %.1f): %d of %d" % (W_EDGE, int(edge.sum()), edge.size),
+                   "tol": 1e-10, "max": worst_edge,
+                   "bar_not_met": "north_star 1e-11 exceeded in %d cell(s)" % len(offenders),
+                   "offenders": offenders[:50]})
+    assert worst_in <= TOL1, worst_in
+    assert worst_edge <= 1e-10, worst_edge
+    assert all(o["W"] > W_EDGE for o in offenders) and len(offenders) <= 16, offenders[:8]
     sg, sr = g.stats(), r.stats()
     for k in ("c2p_fail", "atmo", "w_cap"):
         assert sg[k] == sr[k], (k, sg[k], sr[k])
@@ -332,17 +365,66 @@ def test_config4_c2p_stress_full_size_one_step():
 
 
 def test_config5_bns_quarter_size_one_step():
-    """Config 5 at 128^3 (the oracle's 512^3 state would need ~80 GB of host memory); the
-    512^3 launch configuration itself is exercised by test_config5_full_size_properties."""
+    """Config 5 at 128^3; the 512^3 launch configuration itself is exercised by
+    test_config5_full_size_properties, 256^3 values by test_config5_bns_half_size_one_step."""
     _one_step_case(wl.bns_like(128))
 
 
-@pytest.mark.skipif(__import__("os").environ.get("GRMHD_TEST_512") != "1",
-                    reason="512^3 (88 GB workspace, ~30 GB of host arrays): set GRMHD_TEST_512=1")
-def test_config5_full_size_properties():
-    """512^3 RK4: properties that hold at any size -- finite state, no con2prim failure, the
-    densitised rest mass sum(sqrt(gamma) D) conserved to round-off on the periodic block."""
+def _free_gb():
     import torch
+    free, _ = torch.cuda.mem_get_info()
+    try:
+        host = __import__("psutil").virtual_memory().available
+    except Exception:
+        host = 0
+    return free / 2 ** 30, host / 2 ** 30
+
+
+def test_config5_bns_half_size_one_step():
+    """Config 5 at 256^3, the largest size whose oracle state a 64 GB host holds comfortably:
+    VALUES against the oracle after one RK4 step.  The hydro rows meet 1e-11.  The B rows are
+    curl A of a smooth potential: a rounding difference eps |A| in the evolved A_i becomes
+    eps |A| / (dx |B|) in B, which grows with resolution for a fixed spectrum (5.8e-13 at 32^3,
+    9.0e-12 at 128^3), so B is asserted through what the method evolves -- A_i to 1e-11 -- and
+    bounded by kappa_B * 1e-11 with kappa_B = 4 max|A| / (dx max|B~|) from the data."""
+    dev_gb, host_gb = _free_gb()
+    if dev_gb < 40 or host_gb < 40:
+        pytest.skip("needs 40 GB of device and of host memory")
+    w = wl.bns_like(256)
+    r, g = make_ref(w), make_gpu(w)
+    r.step(1, w.cfl)
+    g.step(1, w.cfl)
+    errs = cons_errors(to_np(g.get_cons()), r.get_cons())
+    eA = _A_err(g, r)
+    Ar, Bf = r.get_vecpot(), r.get_bface()
+    kappa = 4.0 * max(np.abs(a).max() for a in Ar) / (min(w.dx) * max(np.abs(b).max() for b in Bf))
+    REPORT.append({"case": w.name + " one step", "tol": TOL1, "max": max(errs.values()),
+                   "errs": {k: float(v) for k, v in errs.items()}, "A": eA, "kappa_B": float(kappa)})
+    for k in ("D", "Sx", "Sy", "Sz", "tau"):
+        assert errs[k] <= TOL1, errs
+    assert eA <= TOL1, eA
+    for k in ("Bx", "By", "Bz"):
+        assert errs[k] <= max(TOL1, kappa * TOL1), (errs, kappa)
+    sg, sr = g.stats(), r.stats()
+    for k in ("c2p_fail", "atmo", "w_cap"):
+        assert sg[k] == sr[k], (k, sg[k], sr[k])
+    g.close()
+
+
+def test_config5_full_size_properties():
+    """512^3 RK4 (the BASELINE size; ~150 GB of device memory, ~30 GB of host arrays): properties
+    that hold at any size -- finite state, no con2prim failure, the densitised rest mass
+    sum(sqrt(gamma) D) conserved to round-off on the periodic block.  Runs whenever the device
+    and the host have the memory; skipped on memory, not on an environment variable."""
+    import torch
+    from paper_2406_11669_b200 import binding
+    w0 = wl.bns_like(8)
+    need = binding.lib().grmhd_workspace_bytes(512, 512, 512, 3, __import__("ctypes").byref(
+        binding.make_opts(**w0.opts))) / 2 ** 30
+    dev_gb, host_gb = _free_gb()
+    if dev_gb < need + 12 or host_gb < 45:
+        pytest.skip(f"needs {need + 12:.0f} GB of device memory and 45 GB of host memory "
+                    f"(free: {dev_gb:.0f} / {host_gb:.0f})")
     w = wl.make(4)
     g = make_gpu(w)
     I = (slice(3, -3),) * 3
@@ -377,6 +459,39 @@ def test_bns_100_substeps_smooth():
     r.step(25, w.cfl)
     g.step(25, w.cfl)
     _assert_cons(to_np(g.get_cons()), r.get_cons(), TOL100, "bns 25 RK4 steps")
+
+
+# Full-length runs at reduced size with the same generators.  These are NOT smooth:
+# every pressure fix, atmosphere reset or failed recovery is a switch that one ulp can flip, after
+# which the two runs follow different (equally valid) discrete histories.  What is asserted is
+# what such runs support -- same number of steps, finite state, event counters that agree to
+# within the flips, a drift bound from the measurement -- and the measured drift is reported.
+@pytest.mark.parametrize("name,nsteps,drift_bound,count_rtol", [
+    ("kerr", 100, 1e-9, 0.0),        # smooth accretion blob: 4.4e-11 measured, counters identical
+    ("blast", 200, 0.1, 2e-3),       # strong shock + 1 % pressure fixes: 1.7e-2 measured
+    ("stress", 20, None, 1e-2),      # leaves the recovery's domain (1.9 M failures): counters only
+])
+def test_full_length_runs_at_64_cubed(name, nsteps, drift_bound, count_rtol):
+    w = {"kerr": wl.kerr_blob, "blast": wl.blast, "stress": wl.c2p_stress}[name](64)
+    r, g = make_ref(w), make_gpu(w)
+    r.step(nsteps, w.cfl)
+    g.step(nsteps, w.cfl)
+    Ug = to_np(g.get_cons())
+    errs = cons_errors(Ug, r.get_cons())
+    sg, sr = g.stats(), r.stats()
+    REPORT.append({"case": f"{w.name} x {nsteps} steps (drift, reported)", "tol": drift_bound,
+                   "max": float(max(errs.values())), "errs": {k: float(v) for k, v in errs.items()},
+                   "counters_gpu": {k: sg[k] for k in ("c2p_fail", "p_fix", "atmo", "w_cap")},
+                   "counters_ref": {k: sr[k] for k in ("c2p_fail", "p_fix", "atmo", "w_cap")},
+                   "t_gpu": sg["t"], "t_ref": sr["t"]})
+    assert sg["steps"] == sr["steps"] == nsteps and sg["rc"] == 0 and sr["rc"] == 0
+    assert all(np.isfinite(u).all() for u in Ug)
+    for k in ("c2p_fail", "p_fix", "atmo", "w_cap"):
+        assert abs(sg[k] - sr[k]) <= count_rtol * max(sr[k], 1), (k, sg[k], sr[k])
+    np.testing.assert_allclose(sg["t"], sr["t"], rtol=1e-3 if count_rtol else 1e-12)
+    if drift_bound is not None:
+        assert max(errs.values()) <= drift_bound, errs
+    g.close()
 
 
 def test_cuda_graph_step_is_bit_identical_to_eager():
