@@ -13,6 +13,7 @@
 #include "kernels_flux.cuh"
 #include "flux_tma.cuh"
 #include "flux_xrow.cuh"
+#include "flux_xflat.cuh"
 #include "emf_uct.cuh"
 #include "kernels_batch.cuh"
 
@@ -437,8 +438,24 @@ int launch_flux_tma(grmhd* h) {
   return h->E.emf ? launch_flux_tma_v<D, RECON, true>(h) : launch_flux_tma_v<D, RECON, false>(h);
 }
 
+// x fluxes: blocks of 128 consecutive array positions swept in memory order (flux_xflat.cuh)
+template <int RECON>
+int launch_flux_xflat(grmhd* h) {
+  const Geom& g = h->g;
+  const int ap = apron_width(h);
+  const long long ipp = xf_items_per_plane(g, ap);
+  const long long nblk = ipp * (g.nz + 2 * ap);
+  if (h->E.emf)
+    k_flux_xflat<RECON, true><<<(unsigned)nblk, XF_THREADS, 0, h->s>>>(h->base, g, h->E, ap, (int)ipp);
+  else
+    k_flux_xflat<RECON, false><<<(unsigned)nblk, XF_THREADS, 0, h->s>>>(h->base, g, h->E, ap, (int)ipp);
+  h->launches++;
+  return GRMHD_OK;
+}
+
 template <int D, int RECON>
 int launch_flux_dr(grmhd* h) {
+  if (D == 0 && h->flux_impl == 1) return launch_flux_xflat<RECON>(h);
   if (D != 0 && h->flux_impl == 1 && h->tma_ok && h->g.nx >= 32) {
     if constexpr (D != 0) return launch_flux_tma<D, RECON>(h);
   }

@@ -1,0 +1,54 @@
+#!/usr/bin/env python
+"""Mutation check of the oracle pins (test infrastructure; `python tests/mutation_check.py [word ...]`).
+
+Applies one plausible mistake at a time to a COPY of the repository (under the system temp
+directory), rebuilds the oracle there, runs the CPU suite (`-m "not gpu"`) and prints which tests
+turn red.  A mistake that leaves the suite green is a hole in the pins.  The table this printed for
+the committed pins is in DESIGN.md ("Pins of the oracle").  Do not run it beside another OpenMP job:
+two oversubscribed OpenMP runs spin in each other's barriers.
+"""
+import os, shutil, subprocess, sys, tempfile
+SRC=os.path.dirname(os.path.dirname(os.path.abspath(__file__))); DST=os.path.join(tempfile.gettempdir(), "grmhd_mutation_check")
+if os.path.exists(DST): shutil.rmtree(DST)
+shutil.copytree(SRC, DST, ignore=shutil.ignore_patterns(".git","gpurun_out","_work","*.ncu-rep","__pycache__"))
+cpp=os.path.join(DST,"oracle/grmhd_ref.cpp")
+orig=open(cpp).read()
+M=[
+ ("maxspeed over padded range", "      for (int k = 0; k < nz; k++)\n        for (int j = 0; j < ny; j++)\n          for (int i = 0; i < nx; i++) {\n            const size_t c = idx(i, j, k);\n            const Metric M = cell_metric(c);\n            double gu[3][3];",
+                                "      for (int k = -1; k < nz + 1; k++)\n        for (int j = -1; j < ny + 1; j++)\n          for (int i = -1; i < nx + 1; i++) {\n            const size_t c = idx(i, j, k);\n            const Metric M = cell_metric(c);\n            double gu[3][3];"),
+ ("dt: max over directions", "    double dtm = INFINITY;\n    for (int d = 0; d < 3; d++) dtm = std::min(dtm, dx[d] / maxspeed[d]);", "    double dtm = 0;\n    for (int d = 0; d < 3; d++) dtm = std::max(dtm, dx[d] / maxspeed[d]);"),
+ ("dt: speed of wrong shift component", "lam[0] = M.alpha * (vd * (1.0 - a2) - root) / den - M.beta[d];\n  lam[1] = M.alpha * (vd * (1.0 - a2) + root) / den - M.beta[d];", "lam[0] = M.alpha * (vd * (1.0 - a2) - root) / den - M.beta[(d + 1) % 3];\n  lam[1] = M.alpha * (vd * (1.0 - a2) + root) / den - M.beta[(d + 1) % 3];"),
+ ("step_until: no clipping", "    if (dt > t_end - h->t) dt = t_end - h->t;\n", ""),
+ ("RK2: weights 0.25/0.75", "y[q] = 0.5 * Y0[r][q] + 0.5 * (y[q] + h * k2[r][q]);", "y[q] = 0.25 * Y0[r][q] + 0.75 * (y[q] + h * k2[r][q]);"),
+ ("RK3: 0.75/0.25 swapped", "y[q] = 0.75 * Y0[r][q] + 0.25 * (y[q] + h * k2[r][q]);", "y[q] = 0.25 * Y0[r][q] + 0.75 * (y[q] + h * k2[r][q]);"),
+ ("RK3: 1/3,2/3 swapped", "y[q] = (1.0 / 3.0) * Y0[r][q] + (2.0 / 3.0) * (y[q] + h * k3[r][q]);", "y[q] = (2.0 / 3.0) * Y0[r][q] + (1.0 / 3.0) * (y[q] + h * k3[r][q]);"),
+ ("RK4: missing factor 2 on k3", "(k1[r][q] + 2.0 * k2[r][q] + 2.0 * k3[r][q] + k4[r][q])", "(k1[r][q] + 2.0 * k2[r][q] + k3[r][q] + k4[r][q]) * (6.0 / 5.0)"),
+ ("RK4: third stage half step", "for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], h, k3[r], Y(r));", "for (int r = 0; r < 9; r++) axpby(1.0, Y0[r], 0.5 * h, k3[r], Y(r));"),
+ ("A_i ghost: copy instead of linear extrapolation", "                  2.0 * q[idx(J[0], J[1], J[2])] - q[idx(K2[0], K2[1], K2[2])];", "                  q[idx(J[0], J[1], J[2])];"),
+ ("face floors: no velocity cap", "  if (v2 > v2max) {\n    const double f = std::sqrt(v2max / v2);\n    for (int i = 0; i < 3; i++) P[1 + i] *= f;\n  }", ""),
+ ("face floors: cap in the flat norm", "    for (int j = 0; j < 3; j++) v2 += M.g[i][j] * P[1 + i] * P[1 + j];\n  const double v2max", "    for (int j = 0; j < 3; j++) v2 += (i == j) * P[1 + i] * P[1 + j];\n  const double v2max"),
+ ("B~0: sqrt(gamma) dropped", "h->B0[d][c] = 0.5 * (h->sqrtg_cell(cm) * Bin[cm] + h->sqrtg_cell(c) * Bin[c]);", "h->B0[d][c] = 0.5 * (Bin[cm] + Bin[c]);"),
+ ("B~0: sqrt(gamma) of the wrong cell", "h->B0[d][c] = 0.5 * (h->sqrtg_cell(cm) * Bin[cm] + h->sqrtg_cell(c) * Bin[c]);", "h->B0[d][c] = 0.5 * (h->sqrtg_cell(c) * Bin[cm] + h->sqrtg_cell(c) * Bin[c]);"),
+ ("flatten: offset 0.7", "const double f = 10.0 * (dp1 / dp2 - 0.75);", "const double f = 10.0 * (dp1 / dp2 - 0.7);"),
+ ("flatten: slope 5", "const double f = 10.0 * (dp1 / dp2 - 0.75);", "const double f = 5.0 * (dp1 / dp2 - 0.75);"),
+ ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
+ ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
+ ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("HLLE: cmax/cmin swapped on the fluxes", "Fhat[r] = (cmin * GR + cmax * GL - cmax * cmin * (UR[r] - UL[r])) / (cmax + cmin);", "Fhat[r] = (cmax * GR + cmin * GL - cmax * cmin * (UR[r] - UL[r])) / (cmax + cmin);"),
+]
+res={}
+only=sys.argv[1:] 
+for name,a,b in M:
+    if only and not any(o in name for o in only): continue
+    if orig.count(a)!=1:
+        res[name]="PATTERN NOT FOUND x%d"%orig.count(a); print(name,res[name],flush=True); continue
+    open(cpp,"w").write(orig.replace(a,b))
+    so=os.path.join(DST,"oracle/libgrmhd_ref.so")
+    if os.path.exists(so): os.remove(so)
+    p=subprocess.run([sys.executable,"-m","pytest","tests","-q","-m","not gpu","-p","no:cacheprovider","--tb=no","-k","not multirank and not abi"],cwd=DST,capture_output=True,text=True)
+    failed=[l.split(" ")[1] for l in p.stdout.splitlines() if l.startswith("FAILED")]
+    res[name]=failed; print(name,"->",failed,flush=True)
+open(cpp,"w").write(orig)
+holes=[k for k,v in res.items() if not v]
+print("holes:", holes)
+sys.exit(1 if holes else 0)

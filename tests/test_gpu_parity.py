@@ -371,7 +371,10 @@ def test_config5_bns_quarter_size_one_step():
 
 
 def _free_gb():
+    import gc
     import torch
+    gc.collect()
+    torch.cuda.empty_cache()      # blocks cached from earlier tests are not "in use"
     free, _ = torch.cuda.mem_get_info()
     try:
         host = __import__("psutil").virtual_memory().available

@@ -52,3 +52,22 @@ def test_second_step_amplifies_one_ulp_on_the_bns_block():
         errs.append(max(cons_errors(b.get_cons(), a.get_cons()).values()))
     assert errs[0] < 1e-12 and errs[1] > 3.0 * errs[0], errs
     assert a.stats()["p_fix"] > 1000
+
+
+def test_blast_history_is_chaotic_under_one_ulp():
+    """The 48^3 cylindrical blast over 50 RK3 steps (PPM + flattening, ~1 % of the cell-substeps
+    pressure-fixed): two ORACLE runs whose inputs differ by one ulp end 4e-3 apart in the parity
+    norm and with different pressure-fix counts (2e-2 after 200 steps at 64^3).  Every pressure
+    fix is a switch; once one flips the two runs follow different, equally valid discrete
+    histories.  This is why the full-length GPU run of the blast is compared through its step
+    count, counters to a relative 2e-3 and a reported drift -- and why 1e-9 after 100 steps is
+    asserted on smooth data only (north_star)."""
+    w = wl.blast(48)
+    a, b = make_ref(w), make_ref(_perturbed(w))
+    a.step(50, w.cfl)
+    b.step(50, w.cfl)
+    e = max(cons_errors(b.get_cons(), a.get_cons()).values())
+    sa, sb = a.stats(), b.stats()
+    assert e > 1e-6, e
+    assert sa["p_fix"] > 100000 and abs(sa["p_fix"] - sb["p_fix"]) <= 2e-3 * sa["p_fix"]
+    assert sa["c2p_fail"] == sb["c2p_fail"] == 0
