@@ -23,7 +23,7 @@ namespace gk {
 constexpr int XF_THREADS = XF_NTHREADS;
 constexpr int XF_VALID = XF_THREADS - 3;  // faces per block: threads 2 .. 126
 #ifndef XF_MINB
-#define XF_MINB 4
+#define XF_MINB 5
 #endif
 
 // faces of one z-plane: rows j in [-ap, ny + ap), flat offsets o = (j + ap) * sy + (x index)
