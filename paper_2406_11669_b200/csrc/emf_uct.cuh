@@ -30,11 +30,11 @@ __device__ __forceinline__ double uct_limit(double q, double qm, double qp) {
 __device__ __forceinline__ void uct_recon6(const double s[6], double& L, double& R) {
   const double d0 = s[1] - s[0], d1 = s[2] - s[1], d2 = s[3] - s[2], d3 = s[4] - s[3],
                d4 = s[5] - s[4];
-  const double m1 = ft_slope(d0, d1), m2 = ft_slope(d1, d2), m3 = ft_slope(d2, d3),
-               m4 = ft_slope(d3, d4);
-  const double i12 = 0.5 * (s[1] + s[2]) - (m2 - m1) * (1.0 / 6.0);
-  const double i23 = 0.5 * (s[2] + s[3]) - (m3 - m2) * (1.0 / 6.0);
-  const double i34 = 0.5 * (s[3] + s[4]) - (m4 - m3) * (1.0 / 6.0);
+  const double m1 = ft_slope2(d0, d1), m2 = ft_slope2(d1, d2), m3 = ft_slope2(d2, d3),
+               m4 = ft_slope2(d3, d4);
+  const double i12 = ft_iface(s[1], s[2], m1, m2);
+  const double i23 = ft_iface(s[2], s[3], m2, m3);
+  const double i34 = ft_iface(s[3], s[4], m3, m4);
   L = uct_limit<true>(s[2], i12, i23);   // q^+ of the lower cell
   R = uct_limit<false>(s[3], i23, i34);  // q^- of the upper cell
 }

@@ -30,15 +30,22 @@ __device__ __forceinline__ double ft_sel(bool c, double a, double b) {
   return r;
 }
 
-// G8(a): monotonised-central slope from the two one-sided differences.  For same-signed
-// dm, dp the candidates d = (dp+dm)/2 and 2 min(|dp|,|dm|) carry the sign of d already; if
-// one of them is zero so is the candidate chosen, so "dp dm > 0" reduces to a sign-bit test.
-__device__ __forceinline__ double ft_slope(double dm, double dp) {
-  const double d = 0.5 * (dp + dm);
+// G8(a): TWICE the monotonised-central slope from the two one-sided differences (the factor 2
+// is an exact scaling: it saves the halving of the central difference and is undone by the 1/12
+// of ft_iface).  For same-signed dm, dp the candidates dp+dm and 4 min(|dp|,|dm|) carry the sign
+// of the slope already; if one of them is zero so is the candidate chosen, so "dp dm > 0"
+// reduces to a sign-bit test.
+__device__ __forceinline__ double ft_slope2(double dm, double dp) {
+  const double s = dp + dm;
   const double m = fabs(dp) < fabs(dm) ? dp : dm;
-  const double m2 = m + m;
-  const double r = fabs(d) < fabs(m2) ? d : m2;
+  const double m4 = 4.0 * m;
+  const double r = fabs(s) < fabs(m4) ? s : m4;
   return ft_opposite(dp, dm) ? 0.0 : r;
+}
+// G8(b): 4th-order interface value between cells (qa | qb) from their doubled slopes:
+// (qa + qb)/2 - (dm_b - dm_a)/6
+__device__ __forceinline__ double ft_iface(double qa, double qb, double s2a, double s2b) {
+  return 0.5 * (qa + qb) - (s2b - s2a) * (1.0 / 12.0);
 }
 
 // G8(c, d) on the two interface values of a cell: flatten (f = 0 leaves the values untouched
@@ -72,7 +79,7 @@ template <int RECON>
 struct FtMarch {
   double qa, qb;  // q_c, q_{c+1}
   double dl;      // q_c - q_{c-1}
-  double s0;      // PPM: limited slope of cell c
+  double s0;      // PPM: twice the limited slope of cell c
   double il;      // PPM: interface value at c - 1/2
   double qpp;     // q^+ of the previous cell (left state of the next face to be stored)
   // q0..q3 = cells c-2, c-1, c, c+1 where c is the first cell to be processed
@@ -83,9 +90,9 @@ struct FtMarch {
       s0 = 0.0; il = 0.0;
     } else {
       const double d01 = q1 - q0;
-      const double dmA = ft_slope(d01, dl);
-      s0 = ft_slope(dl, q3 - q2);
-      il = 0.5 * (q1 + q2) - (s0 - dmA) * (1.0 / 6.0);
+      const double dmA = ft_slope2(d01, dl);
+      s0 = ft_slope2(dl, q3 - q2);
+      il = ft_iface(q1, q2, dmA, s0);
     }
   }
   // process cell c given qn = q_{c+2} and the flattening coefficient f of cell c
@@ -98,8 +105,8 @@ struct FtMarch {
       qm = fma(-0.5, s, qa);
       qp = fma(0.5, s, qa);
     } else {
-      const double dmn = ft_slope(dr, qn - qb);                        // slope of cell c+1
-      const double ir = 0.5 * (qa + qb) - (dmn - s0) * (1.0 / 6.0);  // interface c + 1/2, G8(b)
+      const double dmn = ft_slope2(dr, qn - qb);       // (doubled) slope of cell c+1
+      const double ir = ft_iface(qa, qb, s0, dmn);      // interface c + 1/2, G8(b)
       qm = il; qp = ir;
       ft_parabola<RECON == 2>(qa, f, anyf, qm, qp);
       s0 = dmn; il = ir;
@@ -110,11 +117,14 @@ struct FtMarch {
 
 // G8(c): flattening coefficient of a cell from p_{c-2}, p_{c-1}, p_{c+1}, p_{c+2} and the
 // normal velocities v_{c-1}, v_{c+1}
+// Called by whole warps: where no lane sees the shock switch the coefficient is 0 without the
+// division.
 __device__ __forceinline__ double ft_flatten(double pm2, double pm1, double pp1, double pp2,
                                              double vm1, double vp1) {
   const double dp1 = pp1 - pm1;
-  const double dp2 = pp2 - pm2;
   const bool on = fabs(dp1) > 0.33 * ft_min(pp1, pm1) && vm1 > vp1;
+  if (!__any_sync(0xffffffffu, on)) return 0.0;
+  const double dp2 = pp2 - pm2;
   const bool z = dp2 == 0.0;
   const double r = ft_rcp(z ? 1.0 : dp2);
   double f = 10.0 * fma(dp1, r, -0.75);
@@ -122,22 +132,6 @@ __device__ __forceinline__ double ft_flatten(double pm2, double pm1, double pp1,
   f = z ? 1.0 : f;
   return on ? f : 0.0;
 }
-
-// ... marching over p_{c-2..c+2}, v_{c-1}, v_{c+1}
-struct FtFlat {
-  double pm2, pm1, p0, pp1, vm1, v0;
-  __device__ __forceinline__ void init(double a, double b, double c, double d, double va,
-                                       double vb) {
-    pm2 = a; pm1 = b; p0 = c; pp1 = d; vm1 = va; v0 = vb;
-  }
-  // pn = p_{c+2}, vn = v_{c+1}
-  __device__ __forceinline__ double step(double pn, double vn) {
-    const double f = ft_flatten(pm2, pm1, pp1, pn, vm1, vn);
-    pm2 = pm1; pm1 = p0; p0 = pp1; pp1 = pn;
-    vm1 = v0; v0 = vn;
-    return f;
-  }
-};
 
 // ---- static face metric ----------------------------------------------------------------------
 struct FaceMet {
@@ -161,17 +155,28 @@ __device__ __forceinline__ FaceMet face_met(const double v[NFM]) {
 // ---- one side of a face ----------------------------------------------------------------------
 // R5 (floors, velocity cap) on the reconstructed state, then U = (D, S_j, tau, B^t1, B^t2) of
 // eqs (20)-(22), the coordinate flux G = alpha F^D of eq. (18) (the alpha: reading G10) and the
-// speeds of R6 / G9 over one denominator:
-//   a^2 = N/Dn, N = Gamma p e + b^2 (rho h - Gamma p), Dn = rho h e, e = rho h + b^2
-//   lambda_pm = alpha (v^d (Dn-N) +- sqrt(N (1-v^2) (g^dd (Dn - v^2 N) - (v^d)^2 (Dn-N))))
-//               / (Dn - v^2 N) - beta^d
+// speeds of R6 / G9.  Written for a low FP64 instruction count (the kernels run against the
+// power cap: every instruction counts):
+//   * S_j in the form of eq. (38), S_j = (z + B^2) v_j - (B^i v_i) B_j with z = rho h W^2
+//     (PAPER.md:268), which needs neither b_j nor alpha b^0; likewise
+//     tau = (z + B^2) - (p + b^2/2) - D   since (rho h + b^2) W^2 - (alpha b^0)^2 = z + B^2;
+//   * b_j alpha B^d / W = alpha B^d (B_j / W^2 + (B^i v_i) v_j)  and  alpha b^0 alpha B^d / W =
+//     alpha B^d (B^i v_i)  (eq. 37 with alpha b^0 = W B^i v_i, eq. 13);
+//   * B_j = gamma_jk B^k with the normal-field part gamma_jD B^D formed once per face (gBn: the
+//     staggered normal field is the same on both sides, G6);
+//   * the speeds over one denominator:
+//       a^2 = N/Dn, N = Gamma p e + b^2 (rho h - Gamma p), Dn = rho h e, e = rho h + b^2
+//       lambda_pm = alpha (v^d (Dn-N) +- sqrt(N (1-v^2) (g^dd (Dn - v^2 N) - (v^d)^2 (Dn-N))))
+//                   / (Dn - v^2 N) - beta^d
 // Rows: 0 D, 1-3 S_j, 4 tau, 5 and 6 the transverse B^{(D+1)%3}, B^{(D+2)%3}.
-// vt (optional): v~^{(D+1)%3}, v~^{(D+2)%3} for eq. (33).
+// Bt1, Bt2 = those transverse components, Bn = B^D; vt (optional): v~^{(D+1)%3}, v~^{(D+2)%3}
+// for eq. (33).
 template <int D>
 __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double vz, double p,
-                                        double Bx, double By, double Bz, const Met& M,
-                                        double gdd, const Eos& E, double U[7], double Gf[7],
-                                        double& lm, double& lp, double* vt = nullptr) {
+                                        double Bt1, double Bt2, double Bn, const double gBn[3],
+                                        const Met& M, double gdd, const Eos& E, double U[7],
+                                        double Gf[7], double& lm, double& lp,
+                                        double* vt = nullptr) {
   rho = rho < E.rho_atm ? E.rho_atm : rho;
   p = p < E.p_floor ? E.p_floor : p;
   double vlx, vly, vlz;
@@ -183,46 +188,56 @@ __device__ __forceinline__ void ft_side(double rho, double vx, double vy, double
     lower(M, vx, vy, vz, vlx, vly, vlz);
     v2 = vlx * vx + vly * vy + vlz * vz;
   }
+  // B_j: transverse part here, normal part from gBn
+  const double Bx = D == 0 ? Bn : (D == 1 ? Bt2 : Bt1);
+  const double By = D == 1 ? Bn : (D == 2 ? Bt2 : Bt1);
+  const double Bz = D == 2 ? Bn : (D == 0 ? Bt2 : Bt1);
   double Blx, Bly, Blz;
-  lower(M, Bx, By, Bz, Blx, Bly, Blz);
+  if (D == 0) {
+    Blx = fma(M.gxz, Bz, fma(M.gxy, By, gBn[0]));
+    Bly = fma(M.gyz, Bz, fma(M.gyy, By, gBn[1]));
+    Blz = fma(M.gzz, Bz, fma(M.gyz, By, gBn[2]));
+  } else if (D == 1) {
+    Blx = fma(M.gxz, Bz, fma(M.gxx, Bx, gBn[0]));
+    Bly = fma(M.gyz, Bz, fma(M.gxy, Bx, gBn[1]));
+    Blz = fma(M.gzz, Bz, fma(M.gxz, Bx, gBn[2]));
+  } else {
+    Blx = fma(M.gxy, By, fma(M.gxx, Bx, gBn[0]));
+    Bly = fma(M.gyy, By, fma(M.gxy, Bx, gBn[1]));
+    Blz = fma(M.gyz, By, fma(M.gxz, Bx, gBn[2]));
+  }
   const double B2 = Blx * Bx + Bly * By + Blz * Bz;
-  const double Bv = Bx * vlx + By * vly + Bz * vlz;
+  const double Bv = Bx * vlx + By * vly + Bz * vlz;   // B^i v_i
   const double iW2 = 1.0 - v2;
   const double W = ft_rsqrt(iW2);
-  const double iW = iW2 * W;
-  const double ab0 = W * Bv;                 // alpha b^0, eq. (13)
-  const double b2 = (B2 + ab0 * ab0) * iW2;  // eq. (13)
-  const double blx = Blx * iW + ab0 * vlx;   // b_i, eq. (37)
-  const double bly = Bly * iW + ab0 * vly;
-  const double blz = Blz * iW + ab0 * vlz;
-  const double rhoh = rho + E.GoGm1 * p;     // eq. (46) with h = 1 + eps + p/rho
-  const double e = rhoh + b2;
-  const double eW2 = e * W * W;
-  const double ptot = p + 0.5 * b2;
+  const double rhoh = rho + E.GoGm1 * p;        // eq. (46) with h = 1 + eps + p/rho
+  const double z = rhoh * (W * W);              // eq. (36)
+  const double b2 = fma(B2, iW2, Bv * Bv);      // eq. (13): b^2 = B^2/W^2 + (B^i v_i)^2
+  const double X = z + B2;
+  const double ptot = fma(0.5, b2, p);
   U[0] = rho * W;
-  U[1] = eW2 * vlx - ab0 * blx;
-  U[2] = eW2 * vly - ab0 * bly;
-  U[3] = eW2 * vlz - ab0 * blz;
-  U[4] = eW2 - ptot - ab0 * ab0 - U[0];
+  U[1] = X * vlx - Bv * Blx;                    // eq. (38)
+  U[2] = X * vly - Bv * Bly;
+  U[3] = X * vlz - Bv * Blz;
+  U[4] = X - ptot - U[0];
   const double vtx = M.a * vx - M.bx, vty = M.a * vy - M.by, vtz = M.a * vz - M.bz;
   const double vtd = D == 0 ? vtx : (D == 1 ? vty : vtz);
   const double vd = D == 0 ? vx : (D == 1 ? vy : vz);
-  const double Bd = D == 0 ? Bx : (D == 1 ? By : Bz);
-  const double aBdW = M.a * Bd * iW;
+  const double aBd = M.a * Bn;
+  const double c1 = aBd * iW2, c2 = aBd * Bv;
   const double ap = M.a * ptot;
   Gf[0] = U[0] * vtd;
-  Gf[1] = U[1] * vtd - blx * aBdW + (D == 0 ? ap : 0.0);
-  Gf[2] = U[2] * vtd - bly * aBdW + (D == 1 ? ap : 0.0);
-  Gf[3] = U[3] * vtd - blz * aBdW + (D == 2 ? ap : 0.0);
-  Gf[4] = U[4] * vtd + ap * vd - ab0 * aBdW;
-  const double B1 = D == 0 ? By : (D == 1 ? Bz : Bx);
-  const double B2t = D == 0 ? Bz : (D == 1 ? Bx : By);
+  Gf[1] = U[1] * vtd - fma(c2, vlx, c1 * Blx) + (D == 0 ? ap : 0.0);
+  Gf[2] = U[2] * vtd - fma(c2, vly, c1 * Bly) + (D == 1 ? ap : 0.0);
+  Gf[3] = U[3] * vtd - fma(c2, vlz, c1 * Blz) + (D == 2 ? ap : 0.0);
+  Gf[4] = fma(U[4], vtd, fma(ap, vd, -c2));
   const double vt1 = D == 0 ? vty : (D == 1 ? vtz : vtx);
   const double vt2 = D == 0 ? vtz : (D == 1 ? vtx : vty);
   if (vt) { vt[0] = vt1; vt[1] = vt2; }
-  U[5] = B1; U[6] = B2t;
-  Gf[5] = B1 * vtd - Bd * vt1;
-  Gf[6] = B2t * vtd - Bd * vt2;
+  U[5] = Bt1; U[6] = Bt2;
+  Gf[5] = Bt1 * vtd - Bn * vt1;
+  Gf[6] = Bt2 * vtd - Bn * vt2;
+  const double e = rhoh + b2;
   const double Gp = E.Gamma * p;
   const double N = Gp * e + b2 * (rhoh - Gp);
   const double Dn = rhoh * e;
@@ -272,14 +287,17 @@ __device__ __forceinline__ void ft_face(const double qL[FX_NV], const double qR[
                                         const FaceMet& fm, const Eos& E, double out[7],
                                         double w[4]) {
   const double Bn = bf * fm.isg;  // G6
+  // gamma_jD B^D, common to both sides
+  const Met& M = fm.M;
+  const double gBn[3] = {(D == 0 ? M.gxx : (D == 1 ? M.gxy : M.gxz)) * Bn,
+                         (D == 0 ? M.gxy : (D == 1 ? M.gyy : M.gyz)) * Bn,
+                         (D == 0 ? M.gxz : (D == 1 ? M.gyz : M.gzz)) * Bn};
   double UL[7], GL[7], UR[7], GR[7], lmL, lpL, lmR, lpR;
   double vtL[2], vtR[2], apm[2];
-  ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], D == 0 ? Bn : (D == 1 ? qL[6] : qL[5]),
-             D == 1 ? Bn : (D == 2 ? qL[6] : qL[5]), D == 2 ? Bn : (D == 0 ? qL[6] : qL[5]),
-             fm.M, fm.gdd, E, UL, GL, lmL, lpL, UCT ? vtL : nullptr);
-  ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], D == 0 ? Bn : (D == 1 ? qR[6] : qR[5]),
-             D == 1 ? Bn : (D == 2 ? qR[6] : qR[5]), D == 2 ? Bn : (D == 0 ? qR[6] : qR[5]),
-             fm.M, fm.gdd, E, UR, GR, lmR, lpR, UCT ? vtR : nullptr);
+  ft_side<D>(qL[0], qL[1], qL[2], qL[3], qL[4], qL[5], qL[6], Bn, gBn, M, fm.gdd, E, UL, GL, lmL,
+             lpL, UCT ? vtL : nullptr);
+  ft_side<D>(qR[0], qR[1], qR[2], qR[3], qR[4], qR[5], qR[6], Bn, gBn, M, fm.gdd, E, UR, GR, lmR,
+             lpR, UCT ? vtR : nullptr);
   ft_hll(UL, GL, lmL, lpL, UR, GR, lmR, lpR, fm.sg, E.riemann, out, UCT ? apm : nullptr);
   if (UCT) {
     const double cs = apm[0] + apm[1];

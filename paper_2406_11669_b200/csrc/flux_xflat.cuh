@@ -81,14 +81,14 @@ k_flux_xflat(double* __restrict__ base, Geom g, Eos E, int ap, int ipp) {
     double dm[FX_NV], ir[FX_NV];
 #pragma unroll
     for (int v = 0; v < FX_NV; v++) {
-      dm[v] = ft_slope(q[v] - qm1[v], qp1[v] - q[v]);
+      dm[v] = ft_slope2(q[v] - qm1[v], qp1[v] - q[v]);
       sa[v][t + 1] = dm[v];
     }
     __syncthreads();
 #pragma unroll
     for (int v = 0; v < FX_NV; v++) {
       const double dmp = sa[v][t + 2];                                   // slope of cell c+1
-      ir[v] = 0.5 * (q[v] + qp1[v]) - (dmp - dm[v]) * (1.0 / 6.0);       // interface c + 1/2
+      ir[v] = ft_iface(q[v], qp1[v], dm[v], dmp);                        // interface c + 1/2
       sb[v][t + 1] = ir[v];
     }
     __syncthreads();

@@ -39,9 +39,9 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
     qm = fma(-0.5, s, q);
     qp = fma(0.5, s, q);
   } else {  // G8(a)-(d), same arithmetic as FtMarch::step
-    const double dm = ft_slope(dl, dr);
+    const double dm = ft_slope2(dl, dr);
     const double dmp = fx_dn(dm, 1);                             // slope of cell c+1
-    const double ir = 0.5 * (q + qp1) - (dmp - dm) * (1.0 / 6.0);  // interface c + 1/2
+    const double ir = ft_iface(q, qp1, dm, dmp);                 // interface c + 1/2
     qm = fx_up(ir, 1);                                           // interface c - 1/2
     qp = ir;
     ft_parabola<RECON == 2>(q, f, anyf, qm, qp);
