@@ -164,6 +164,8 @@ int grmhd_get_psi(grmhd* h, double* field);
  * "flux_kernel" (1 default: y and z fluxes by the TMA-fed marching kernel, x fluxes with the lanes
  * of a warp along x; 0: lanes along the flux direction in all three directions -- what blocks
  * narrower than 32 cells in x use anyway);
+ * "src_kernel" (1 default: the metric-derivative stencils of the source terms in x and y from a
+ * TMA-staged shared-memory tile; 0: plain loads -- bit-identical results);
  * "graph" (1 default: after one eager step the launch sequence of a step is captured into a
  * CUDA graph and every later step is one cudaGraphLaunch into the handle's stream -- same
  * kernels, same arguments, bit-identical results; any other option or grmhd_set_mask drops the

@@ -20,11 +20,12 @@
 // One __syncthreads per chunk.  Slot reuse: stage n+1 is issued after the barrier of iteration n,
 // i.e. after every thread has finished phase B of chunk n-1, the last reader of that slot.
 // The 2 ap apron columns x < 0, x >= nx (ap = 1 flux-CT, R10; 3 upwind CT, G27) are not 32-wide
-// groups; they go through k_flux_xrow (flux_xrow.cuh, mode 1).
+// groups; they go through k_flux_xrow (flux_xrow.cuh, mode 1), a launch of its own after this
+// one.  (Solved at the end of the first and last group's blocks instead -- where their loads hit
+// L2 -- they cost more: 0.98 against 0.91 ms, the blocks of those groups finish late.)
 #pragma once
-#include <cuda.h>
-
 #include "flux_face.cuh"
+#include "tma.cuh"
 
 namespace gk {
 
@@ -37,6 +38,9 @@ constexpr int FT_SLOTS = FT_NSLOTS;
 #ifndef FT_MINB
 #define FT_MINB 3
 #endif
+#ifndef FT_UCT_MINB
+#define FT_UCT_MINB 3
+#endif
 
 struct FtSmem {
   // ring slots (TMA destinations, dense boxes [field][face][pencil])
@@ -48,47 +52,12 @@ struct FtSmem {
   alignas(8) unsigned long long bar[FT_SLOTS];
 };
 
-// ---- PTX wrappers -------------------------------------------------------------------------
-__device__ __forceinline__ unsigned ft_saddr(const void* p) {
-  return (unsigned)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void ft_mbar_init(unsigned long long* bar, int count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(ft_saddr(bar)), "r"(count));
-}
-__device__ __forceinline__ void ft_mbar_expect(unsigned long long* bar, unsigned bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(ft_saddr(bar)),
-               "r"(bytes)
-               : "memory");
-}
-__device__ __forceinline__ void ft_mbar_wait(unsigned long long* bar, unsigned parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "FT_WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra FT_DONE_%=;\n"
-      "bra FT_WAIT_%=;\n"
-      "FT_DONE_%=:\n"
-      "}\n" ::"r"(ft_saddr(bar)),
-      "r"(parity)
-      : "memory");
-}
-__device__ __forceinline__ void ft_tma_4d(void* dst, const CUtensorMap* tm,
-                                          unsigned long long* bar, int c0, int c1, int c2,
-                                          int c3) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes "
-      "[%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(ft_saddr(dst)),
-      "l"(tm), "r"(ft_saddr(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-      : "memory");
-}
-
 // RECON: 0 minmod, 1 PPM without flattening, 2 PPM with flattening.  D = 1 (y) or 2 (z).
 // grid: x = (groups of 32 along x) * (n_t1 + 2 ap), y = segments of `seglen` faces (a multiple
 // of TC).  UCT (compile time, so that the default kernel keeps its register budget): also store
 // the upwind-CT face rows of F_W.
 template <int D, int RECON, bool UCT>
-__global__ void __launch_bounds__(FT_THREADS, UCT ? 2 : FT_MINB)
+__global__ void __launch_bounds__(FT_THREADS, UCT ? FT_UCT_MINB : FT_MINB)
 k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx, int ap,
            const __grid_constant__ CUtensorMap tmMet, const __grid_constant__ CUtensorMap tmBf) {
   static_assert(D == 1 || D == 2, "x fluxes: k_flux_xrow");

@@ -48,33 +48,17 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
   }
 }
 
-// grid: one warp per (pencil, segment) item: item = pencil * nsd + seg.  With (t0, t1) the
-// transverse axes -- (y, z) for D = x, (x, z) for D = y, (x, y) for D = z -- and `ap` the
-// transverse apron (1 for flux-CT, R10; 3 for the upwind CT, G27):
-//   mode 0: every pencil t0 in [-ap, n_t0 + ap), t1 in [-ap, n_t1 + ap).  The x fluxes; for
-//           D = y, z the lanes then run along y or z with a stride (uncoalesced: small
-//           blocks and option combinations only).
-//   mode 1: only the 2 ap apron columns t0 < 0 and t0 >= n_t0 that the 32-wide groups of
-//           k_flux_tma leave out.
-// UCT (compile time, as in k_flux_tma): also store the upwind-CT face rows of F_W.
+// One item: the warp's 32 lanes are the cells c0 .. c0+31 along D of the pencil (t0, t1) -- with
+// (t0, t1) the transverse axes: (y, z) for D = x, (x, z) for D = y, (x, y) for D = z -- and the
+// lane of cell c solves face c - 1/2.  Faces outside [flo, fhi) are not stored.  Call with whole
+// warps.  UCT (compile time): also store the upwind-CT face rows of F_W.
 template <int D, int RECON, bool UCT>
-__global__ void __launch_bounds__(FX_THREADS, FX_MINB)
-k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems, int ap,
-            int mode) {
+__device__ __forceinline__ void fx_item(double* __restrict__ base, const Geom& g, const Eos& E,
+                                        int c0, int t0, int t1, int flo, int fhi) {
   const int lane = threadIdx.x & 31;
-  const long long nwarp = (long long)gridDim.x * (FX_THREADS / 32);
   const int nD = g.n(D);
-  const int nt0 = D == 0 ? g.ny : g.nx;
-  const int w0 = mode ? 2 * ap : nt0 + 2 * ap;
-  // grid-stride loop over the items (the launch gives every warp one item)
-  for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
-       item < nitems; item += nwarp) {
-  const int seg = (int)(item % nsd);
-  const int row = (int)(item / nsd);
-  const int c = seg * FX_VALID - 3 + lane;  // this lane's cell along D; its face is c - 1/2
+  const int c = c0 + lane;                  // this lane's cell along D; its face is c - 1/2
   const int cc = min(c, nD + G - 1);        // lanes past the last ghost cell reuse it
-  const int q0 = row % w0, t1 = row / w0 - ap;
-  const int t0 = mode ? (q0 < ap ? q0 - ap : nt0 + q0 - ap) : q0 - ap;
   const int idx = (int)(D == 0 ? g.at(cc, t0, t1) : (D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc)));
 
   // ---- cell data of the lane: rho, v^x, v^y, v^z, p and the two transverse B; the static face
@@ -109,7 +93,7 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
   const FaceMet fmet = face_met<D>(mv11);
   double out[7], w[4];
   ft_face<D, UCT>(qL, qR, bfx, fmet, E, out, w);
-  if (lane >= 3 && lane < 3 + FX_VALID && c <= nD) {
+  if (lane >= 3 && lane < 3 + FX_VALID && c >= flo && c < fhi) {
     double* o = fld(base, g, flux_field(D)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
@@ -120,7 +104,30 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
       for (int r = 0; r < 4; r++) ow[r * NPA] = w[r];
     }
   }
-  }  // items
+}
+
+// grid: one warp per (pencil, segment) item: item = pencil * nsd + seg.  `ap` = the transverse
+// apron (1 for flux-CT, R10; 3 for the upwind CT, G27):
+//   mode 0: every pencil t0 in [-ap, n_t0 + ap), t1 in [-ap, n_t1 + ap).  For D = y, z the lanes
+//           then run along y or z with a stride (uncoalesced: small blocks and option
+//           combinations only).
+//   mode 1: only the 2 ap apron columns t0 < 0 and t0 >= n_t0.
+template <int D, int RECON, bool UCT>
+__global__ void __launch_bounds__(FX_THREADS, FX_MINB)
+k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems, int ap,
+            int mode) {
+  const long long nwarp = (long long)gridDim.x * (FX_THREADS / 32);
+  const int nt0 = D == 0 ? g.ny : g.nx;
+  const int w0 = mode ? 2 * ap : nt0 + 2 * ap;
+  // grid-stride loop over the items (the launch gives every warp one item)
+  for (long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
+       item < nitems; item += nwarp) {
+    const int seg = (int)(item % nsd);
+    const int row = (int)(item / nsd);
+    const int q0 = row % w0, t1 = row / w0 - ap;
+    const int t0 = mode ? (q0 < ap ? q0 - ap : nt0 + q0 - ap) : q0 - ap;
+    fx_item<D, RECON, UCT>(base, g, E, seg * FX_VALID - 3, t0, t1, 0, g.n(D) + 1);
+  }
 }
 
 }  // namespace gk

@@ -14,6 +14,7 @@
 #include "flux_tma.cuh"
 #include "flux_xrow.cuh"
 #include "flux_xflat.cuh"
+#include "src_tile.cuh"
 #include "emf_uct.cuh"
 #include "kernels_batch.cuh"
 
@@ -38,6 +39,8 @@ struct grmhd {
   long long launches = 0;
   int ft_conc[18] = {0};  // resident blocks of each k_flux_tma instantiation (0 = not queried)
   CUtensorMap tm_met[3], tm_bf[3];  // 4-D boxes [field][.][.][x] of the ring stages (y, z)
+  CUtensorMap tm_src;               // [10 fields][1][12][36] tile of k_src_tile
+  int src_impl = 1;                 // 1: k_src_tile (TMA-staged x-y stencils), 0: k_src
   bool tma_ok = false;
   int uct_nseg = 16;     // segments of the marching passes along y and z
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
@@ -301,6 +304,8 @@ int set_params(grmhd* h, double cfl, double t_end) {
   return GRMHD_OK;
 }
 
+int launch_src(grmhd* h);
+
 // R13 + R14 + R15 after a change of (U~, A)
 int after_stage(grmhd* h, bool want_speed) {
   const Geom& g = h->g;
@@ -319,8 +324,8 @@ int after_stage(grmhd* h, bool want_speed) {
     CKL("k_post");
   });
   KT(KG_SRC, {
-    k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
-    CKL("k_src");
+    rc = launch_src(h);
+    if (rc) return rc;
   });
   KT(KG_GHOST, {
     rc = fill_ghosts(h, fill_prims());
@@ -387,7 +392,30 @@ bool make_tensor_maps(grmhd* h) {
       if (r != CUDA_SUCCESS) return false;
     }
   }
+  {
+    const cuuint32_t box[4] = {ST_TX, ST_TY, 1, ST_NF};
+    CUresult r = ((EncodeTiledFn)fn)(&h->tm_src, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, h->base, dims,
+                                     strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return false;
+  }
   return true;
+}
+
+// A5 sources of the current primitives into F_SRC
+int launch_src(grmhd* h) {
+  const Geom& g = h->g;
+  if (h->src_impl == 1 && h->tma_ok) {
+    const dim3 grid((g.nx + ST_BX - 1) / ST_BX, (g.ny + ST_BY - 1) / ST_BY, g.nz);
+    k_src_tile<<<grid, dim3(ST_BX, ST_BY, 1), sizeof(SrcTileSmem), h->s>>>(h->base, g, h->E,
+                                                                            h->tm_src);
+    CKL("k_src_tile");
+  } else {
+    k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
+    CKL("k_src");
+  }
+  return GRMHD_OK;
 }
 
 template <int D, int RECON, bool UCT>
@@ -615,9 +643,7 @@ int init_state(grmhd* h) {
   k_post<true, false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
       h->base, nullptr, g, h->E, h->dst, 1);
   CKL("k_post");
-  k_src<<<grd_src(g), dim3(KS_BX, KS_BY, 1), 0, h->s>>>(h->base, g, h->E);
-  CKL("k_src");
-  return GRMHD_OK;
+  return launch_src(h);
 }
 
 }  // namespace
@@ -886,6 +912,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "flux_kernel") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
     h->flux_impl = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "src_kernel") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: src_kernel is 0 or 1");
+    h->src_impl = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "gauge") == 0) {

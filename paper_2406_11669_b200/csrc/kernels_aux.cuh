@@ -304,6 +304,16 @@ __device__ __forceinline__ double d4(const double* __restrict__ q, int c, int sd
   return (8.0 * (q[c + sd] - q[c - sd]) - (q[c + 2 * sd] - q[c - 2 * sd])) * i12dx;
 }
 
+// One axis of R9: d[0..9] = d_a of alpha, beta^x, beta^y, beta^z, gamma_xx .. gamma_zz at the cell.
+// S_a = alpha sqrt(gamma) (C^{ik} d_a gamma_ik - T^{00} alpha d_a alpha + T^0_i d_a beta^i) and
+// the d_a alpha part of S_tau.
+__device__ __forceinline__ void src_axis(const SrcCoef& sc, int a, const double d[10], double asg,
+                                         double S[4], double& St) {
+  const double cg = contract(sc.C, d[4], d[5], d[6], d[7], d[8], d[9]);
+  S[a] = asg * (cg - sc.T00a * d[0] + sc.T0lx * d[1] + sc.T0ly * d[2] + sc.T0lz * d[3]);
+  St -= (a == 0 ? sc.ax : (a == 1 ? sc.ay : sc.az)) * d[0];
+}
+
 // R9 / G11: alpha sqrt(gamma) S for the rows S_x, S_y, S_z, tau at an interior cell
 // (eq. (19) PAPER.md:125 in 3+1 form; metric derivatives PAPER.md:384)
 __device__ __forceinline__ void cell_sources(const double* __restrict__ base, const Geom& g, int c,
@@ -319,18 +329,10 @@ __device__ __forceinline__ void cell_sources(const double* __restrict__ base, co
   for (int a = 0; a < 3; a++) {
     const int sd = a == 0 ? 1 : (a == 1 ? (int)g.sy : (int)g.sz);
     const double w = g.idx[a] * (1.0 / 12.0);
-    const double da = d4(fld(base, g, F_MET + 0), c, sd, w);
-    const double dbx = d4(fld(base, g, F_MET + 1), c, sd, w);
-    const double dby = d4(fld(base, g, F_MET + 2), c, sd, w);
-    const double dbz = d4(fld(base, g, F_MET + 3), c, sd, w);
-    const double cg = contract(sc.C, d4(fld(base, g, F_MET + 4), c, sd, w),
-                               d4(fld(base, g, F_MET + 5), c, sd, w),
-                               d4(fld(base, g, F_MET + 6), c, sd, w),
-                               d4(fld(base, g, F_MET + 7), c, sd, w),
-                               d4(fld(base, g, F_MET + 8), c, sd, w),
-                               d4(fld(base, g, F_MET + 9), c, sd, w));
-    S[a] = asg * (cg - sc.T00a * da + sc.T0lx * dbx + sc.T0ly * dby + sc.T0lz * dbz);
-    St -= (a == 0 ? sc.ax : (a == 1 ? sc.ay : sc.az)) * da;
+    double d[10];
+#pragma unroll
+    for (int f = 0; f < 10; f++) d[f] = d4(fld(base, g, F_MET + f), c, sd, w);
+    src_axis(sc, a, d, asg, S, St);
   }
   S[3] = asg * St;
 }
