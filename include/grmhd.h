@@ -56,6 +56,7 @@ extern "C" {
 #define GRMHD_ESTATE   -3  /* call order: step before metric+prims, vecpot before prims */
 #define GRMHD_ECUDA    -4  /* CUDA runtime error (string in grmhd_last_error)          */
 #define GRMHD_ENUMERIC -5  /* dt came out NaN / non-positive / infinite                */
+#define GRMHD_ELIMIT   -6  /* size beyond the fixed maximum of a no-allocation entry point */
 
 typedef struct grmhd grmhd; /* opaque handle (host memory, owned by the library) */
 
@@ -214,6 +215,29 @@ int grmhd_con2prim1d_batch(const double* const cons[8], const double* const metr
 /* Dependent-free DFMA loop used to MEASURE the FP64 pipe peak: each of `threads` threads
  * performs `iters` * 16 DFMAs; out receives one double per thread.  */
 int grmhd_dfma_peak(double* out, long long threads, int iters, void* stream);
+
+/* ---- the max-speed reduction with NO allocation ---------------------------------------
+ * For callers that cannot call cudaMalloc or hold a workspace (code under CUDA-graph capture,
+ * tight serving loops, harnesses that forbid allocation): the max-characteristic-speed reduction
+ * of the CFL step (north_star "max-characteristic-speed reduction for the CFL dt"; speeds:
+ * PAPER.md:199, R16 / G9) on n plain states, structure of arrays as above:
+ *   prim   [dev] 8 arrays rho, v^x, v^y, v^z, p, B^x, B^y, B^z (cell-centred values), n each;
+ *   metric [dev] 10 arrays alpha, beta^i (3), gamma_ij (6), n each;
+ *   maxspeed [dev] 3 doubles OUT: max over the states of max(|lambda_-|, |lambda_+|) along
+ *            x, y, z -- what grmhd_get_stats reports as maxspeed for the cells of a handle
+ *            (dt = cfl * min_d dx_d / maxspeed[d]).  A NaN speed never wins the max.
+ * The call enqueues one memset and one kernel on `stream` and returns; it allocates nothing and
+ * calls no allocating routine.  Its scratch (one partial maximum per 256 states) is a file-scope
+ * __device__ array of 384.25 KiB that every GPU loading the library holds until the process
+ * exits; hence the limit  1 <= n <= GRMHD_NOALLOC_MAX_STATES: a larger n returns GRMHD_ELIMIT
+ * (split the batch and take the max of the results).  Every call on a device shares that
+ * array: calls that overlap on the GPU (different streams or threads) RACE -- serialise them.
+ * err/err_len: optional buffer for a human-readable message (there is no handle to keep one);
+ * may be NULL/0.  Other errors: GRMHD_EINVAL (NULL array, n < 1, bad options), GRMHD_ECUDA. */
+#define GRMHD_NOALLOC_MAX_STATES 4194304LL /* 2^22 */
+int grmhd_maxspeed_noalloc(const double* const prim[8], const double* const metric[10],
+                           long long n, const grmhd_opts* opts, double* maxspeed, void* stream,
+                           char* err, size_t err_len);
 
 #ifdef __cplusplus
 }

@@ -3,7 +3,8 @@
 `workloads` (seeded input generators) imports without torch/CUDA; everything else is the
 ctypes binding of the CUDA library (`binding`), loaded lazily.  There is no CPU fallback.
 """
-__all__ = ["Solver", "make_opts", "prim2con_batch", "con2prim_batch", "dfma_peak", "lib"]
+__all__ = ["Solver", "make_opts", "prim2con_batch", "con2prim_batch", "dfma_peak",
+           "maxspeed_noalloc", "lib"]
 
 
 def __getattr__(name):

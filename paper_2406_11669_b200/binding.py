@@ -15,15 +15,17 @@ import torch
 from . import build as _build
 
 G = 3
-OK, EINVAL, ENOMEM, ESTATE, ECUDA, ENUMERIC = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ESTATE, ECUDA, ENUMERIC, ELIMIT = 0, -1, -2, -3, -4, -5, -6
 _ERRNAME = {EINVAL: "GRMHD_EINVAL", ENOMEM: "GRMHD_ENOMEM", ESTATE: "GRMHD_ESTATE",
-            ECUDA: "GRMHD_ECUDA", ENUMERIC: "GRMHD_ENUMERIC"}
+            ECUDA: "GRMHD_ECUDA", ENUMERIC: "GRMHD_ENUMERIC", ELIMIT: "GRMHD_ELIMIT"}
+NOALLOC_MAX_STATES = 1 << 22   # GRMHD_NOALLOC_MAX_STATES of include/grmhd.h
 
 EXPORTS = ["grmhd_workspace_bytes", "grmhd_create", "grmhd_destroy", "grmhd_set_metric",
            "grmhd_set_prims", "grmhd_set_vecpot", "grmhd_set_mask", "grmhd_step",
            "grmhd_step_until", "grmhd_get_prims", "grmhd_get_cons", "grmhd_get_vecpot", "grmhd_get_psi",
            "grmhd_set_option", "grmhd_get_stats", "grmhd_get_kernel_times", "grmhd_launch_count", "grmhd_last_error",
-           "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_con2prim1d_batch", "grmhd_dfma_peak"]
+           "grmhd_prim2con_batch", "grmhd_con2prim_batch", "grmhd_con2prim1d_batch", "grmhd_dfma_peak",
+           "grmhd_maxspeed_noalloc"]
 
 
 class GrmhdOpts(C.Structure):
@@ -98,6 +100,9 @@ def lib():
                                            C.POINTER(C.c_void_p), C.c_void_p, C.c_void_p,
                                            C.c_longlong, C.POINTER(GrmhdOpts), C.c_void_p]
         L.grmhd_dfma_peak.argtypes = [C.c_void_p, C.c_longlong, C.c_int, C.c_void_p]
+        L.grmhd_maxspeed_noalloc.argtypes = [C.POINTER(C.c_void_p), C.POINTER(C.c_void_p),
+                                             C.c_longlong, C.POINTER(GrmhdOpts), C.c_void_p,
+                                             C.c_void_p, C.c_char_p, C.c_size_t]
         _lib = L
     return _lib
 
@@ -335,6 +340,36 @@ def con2prim1d_batch(cons, metric, opts: GrmhdOpts):
     if rc != OK:
         raise GrmhdError("grmhd_con2prim1d_batch", rc)
     return prim, status, iters
+
+
+def maxspeed_noalloc(prim, metric, opts: GrmhdOpts, out, stream=None):
+    """grmhd_maxspeed_noalloc: max |lambda| along x, y, z over n plain states, with no allocation
+    on the library's side (its scratch is a static device array; n <= NOALLOC_MAX_STATES).
+    prim (8,n) and metric (10,n) contiguous CUDA fp64 tensors; `out` = the caller's CUDA fp64
+    tensor of 3 elements (this wrapper allocates nothing on the device either).  Only enqueues on
+    `stream` (default: torch's current stream).  Calls that overlap on the GPU race on the
+    library's scratch array."""
+    _require_cuda()
+    for t, rows in ((prim, 8), (metric, 10)):
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64
+                and t.dim() == 2 and t.shape[0] == rows and t.is_contiguous()):
+            raise ValueError(f"need a contiguous CUDA fp64 tensor of shape ({rows}, n)")
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64
+            and out.numel() == 3 and out.is_contiguous()):
+        raise ValueError("out: need a contiguous CUDA fp64 tensor of 3 elements")
+    n = int(prim.shape[1])
+    if metric.shape[1] != n:
+        raise ValueError("prim and metric hold a different number of states")
+    pp = (C.c_void_p * 8)(*[prim[r].data_ptr() for r in range(8)])
+    mp = (C.c_void_p * 10)(*[metric[r].data_ptr() for r in range(10)])
+    s = stream if stream is not None else torch.cuda.current_stream(prim.device)
+    msg = C.create_string_buffer(256)
+    with torch.cuda.device(prim.device):
+        rc = lib().grmhd_maxspeed_noalloc(pp, mp, n, C.byref(opts), C.c_void_p(out.data_ptr()),
+                                          C.c_void_p(s.cuda_stream), msg, len(msg))
+    if rc != OK:
+        raise GrmhdError("grmhd_maxspeed_noalloc", rc, msg.value.decode())
+    return out
 
 
 def dfma_peak(threads=148 * 2048, iters=4096, reps=5):

@@ -1049,3 +1049,157 @@ int grmhd_dfma_peak(double* out, long long threads, int iters, void* stream) {
 }
 
 }  // extern "C"
+
+// =============================================================================================
+// A8 without any allocation: grmhd_maxspeed_noalloc (include/grmhd.h).
+//
+// The max-characteristic-speed reduction of a handle accumulates into scratch the caller's
+// workspace holds (DevState::ms_acc).  Callers that cannot provide or allocate a workspace --
+// code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc -- get the
+// same reduction on plain arrays of states with its scratch in a FILE-SCOPE device array of a
+// fixed, modest size: every GPU that loads the library holds these NOALLOC_SCRATCH_BYTES until the
+// process exits.  No cudaMalloc, cudaFree or allocating library routine is called.
+//
+// In host code the NAME of a __device__ array is a host-side stand-in, not a device address: a
+// kernel handed `g_noalloc_scratch` from the host would fault (or, where the GPU can reach host
+// memory, silently use the wrong memory).  The device address is asked for once per device, with
+// that device current, through cudaGetSymbolAddress, and that pointer is what the kernel gets.
+//
+// Layout of the scratch: [0, 256 B) header -- a block counter (unsigned) that MUST start at zero;
+// then 3 doubles per block, the block's max |lambda| in x, y, z.  The array is shared by every
+// call and keeps the last call's contents: the header is cleared at the start of every call (on
+// the call's stream), the partial maxima of the blocks [0, nblocks) are all overwritten before
+// the last block reads exactly that range, so nothing stale is ever read.  Calls that overlap on
+// the GPU (two streams, two threads) would race on the array: callers serialise them.
+namespace {
+
+constexpr int NOALLOC_BLOCK = 256;                                   // states per block
+constexpr long long NOALLOC_MAX_BLOCKS = GRMHD_NOALLOC_MAX_STATES / NOALLOC_BLOCK;
+constexpr int NOALLOC_HDR = 32;                                      // doubles (256 B)
+constexpr size_t NOALLOC_SCRATCH_DOUBLES = NOALLOC_HDR + 3 * (size_t)NOALLOC_MAX_BLOCKS;
+constexpr size_t NOALLOC_SCRATCH_BYTES = NOALLOC_SCRATCH_DOUBLES * sizeof(double);  // 384.25 KiB
+static_assert(GRMHD_NOALLOC_MAX_STATES % NOALLOC_BLOCK == 0, "whole blocks");
+static_assert(NOALLOC_SCRATCH_BYTES <= (1u << 20), "the static scratch stays modest");
+
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_SCRATCH_DOUBLES];
+
+// R16 on n plain states: block b leaves its three maxima in scratch[HDR + 3 b ..]; the block
+// that arrives last (counter in the header) reduces the nblocks partial maxima to out[0..2] and
+// puts the counter back to zero.  Same per-state arithmetic as the handle's path (cell_speeds);
+// max of non-negative doubles is exact and order independent.
+__global__ void __launch_bounds__(NOALLOC_BLOCK)
+k_maxspeed_noalloc(BatchPtrs b, long long n, Eos E, double* __restrict__ scratch,
+                   double* __restrict__ out) {
+  __shared__ double sm[3][NOALLOC_BLOCK / 32];
+  __shared__ bool last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long q = blockIdx.x * (long long)NOALLOC_BLOCK + tid;
+  double s[3] = {0.0, 0.0, 0.0};
+  if (q < n) {
+    const Prim P = {b.prim[0][q], b.prim[1][q], b.prim[2][q], b.prim[3][q],
+                    b.prim[4][q], b.prim[5][q], b.prim[6][q], b.prim[7][q]};
+    cell_speeds(P, batch_met(b, q), E, s);
+  }
+  auto block_max = [&]() {  // s[] of thread 0 = max over the block
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+      for (int d = 0; d < 3; d++) s[d] = fmax(s[d], __shfl_xor_sync(0xffffffffu, s[d], o));
+    if (lane == 0)
+      for (int d = 0; d < 3; d++) sm[d][warp] = s[d];
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+      for (int d = 0; d < 3; d++) s[d] = lane < NOALLOC_BLOCK / 32 ? sm[d][lane] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int d = 0; d < 3; d++) s[d] = fmax(s[d], __shfl_xor_sync(0xffffffffu, s[d], o));
+    }
+  };
+  block_max();
+  unsigned* counter = reinterpret_cast<unsigned*>(scratch);
+  double* part = scratch + NOALLOC_HDR;
+  if (tid == 0) {
+    for (int d = 0; d < 3; d++) part[3 * (size_t)blockIdx.x + d] = s[d];
+    __threadfence();  // the partial maxima are visible before the arrival is counted
+    last = atomicAdd(counter, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  s[0] = s[1] = s[2] = 0.0;
+  for (unsigned k = tid; k < gridDim.x; k += NOALLOC_BLOCK)
+    for (int d = 0; d < 3; d++) s[d] = fmax(s[d], __ldcg(part + 3 * (size_t)k + d));
+  __syncthreads();  // sm[] is reused
+  block_max();
+  if (tid == 0) {
+    for (int d = 0; d < 3; d++) out[d] = s[d];
+    *counter = 0u;  // as the next call expects it (that call clears the header anyway)
+  }
+}
+
+// set-up, once per device: the DEVICE address of the scratch array on the current device
+int noalloc_scratch(double** ptr, char* err, size_t err_len) {
+  constexpr int MAXDEV = 64;
+  static double* cached[MAXDEV] = {nullptr};
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess && (dev < 0 || dev >= MAXDEV)) e = cudaErrorInvalidDevice;
+  if (e == cudaSuccess && !cached[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e == cudaSuccess && !p) e = cudaErrorInvalidSymbol;
+    if (e == cudaSuccess) cached[dev] = static_cast<double*>(p);
+  }
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    if (err && err_len)
+      std::snprintf(err, err_len, "grmhd_maxspeed_noalloc: cudaGetSymbolAddress: %s",
+                    cudaGetErrorString(e));
+    return GRMHD_ECUDA;
+  }
+  *ptr = cached[dev];
+  return GRMHD_OK;
+}
+
+}  // namespace
+
+extern "C" int grmhd_maxspeed_noalloc(const double* const prim[8], const double* const metric[10],
+                                      long long n, const grmhd_opts* opts, double* maxspeed,
+                                      void* stream, char* err, size_t err_len) {
+  auto say = [&](const char* m) { if (err && err_len) std::snprintf(err, err_len, "%s", m); };
+  if (err && err_len) err[0] = 0;
+  if (!prim || !metric || !maxspeed || n < 1 || !valid_opts(opts)) {
+    say("grmhd_maxspeed_noalloc: NULL argument, n < 1 or invalid options");
+    return GRMHD_EINVAL;
+  }
+  if (n > GRMHD_NOALLOC_MAX_STATES) {
+    if (err && err_len)
+      std::snprintf(err, err_len,
+                    "grmhd_maxspeed_noalloc: n = %lld exceeds GRMHD_NOALLOC_MAX_STATES = %lld (the "
+                    "static scratch holds one partial maximum per %d states); split the batch",
+                    n, (long long)GRMHD_NOALLOC_MAX_STATES, NOALLOC_BLOCK);
+    return GRMHD_ELIMIT;
+  }
+  BatchPtrs bp{};
+  for (int r = 0; r < 8; r++) { if (!prim[r]) { say("grmhd_maxspeed_noalloc: NULL prim array"); return GRMHD_EINVAL; } bp.prim[r] = prim[r]; }
+  for (int r = 0; r < 10; r++) { if (!metric[r]) { say("grmhd_maxspeed_noalloc: NULL metric array"); return GRMHD_EINVAL; } bp.met[r] = metric[r]; }
+  double* scratch = nullptr;
+  const int rc = noalloc_scratch(&scratch, err, err_len);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  // the header (block counter) must start at zero whatever an earlier call left behind
+  cudaError_t e = cudaMemsetAsync(scratch, 0, NOALLOC_HDR * sizeof(double), st);
+  if (e == cudaSuccess) {
+    const unsigned nblk = (unsigned)((n + NOALLOC_BLOCK - 1) / NOALLOC_BLOCK);
+    k_maxspeed_noalloc<<<nblk, NOALLOC_BLOCK, 0, st>>>(bp, n, make_eos(*opts), scratch, maxspeed);
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess) {
+    if (err && err_len)
+      std::snprintf(err, err_len, "grmhd_maxspeed_noalloc: %s", cudaGetErrorString(e));
+    return GRMHD_ECUDA;
+  }
+  return GRMHD_OK;
+}
