@@ -161,7 +161,10 @@ class Solver:
     """One handle of the C ABI.  Inputs: torch tensors (CUDA or pinned/pageable host) or
     numpy arrays, fp64, shapes (nz+6, ny+6, nx+6) / staggered (nz+7, ny+7, nx+7)."""
 
-    def __init__(self, nx, ny, nz, dx, opts: GrmhdOpts, device="cuda:0", stream=None):
+    def __init__(self, nx, ny, nz, dx, opts: GrmhdOpts, device="cuda:0", stream=None,
+                 guard_bytes=0):
+        """guard_bytes > 0 (tests): that many bytes of 0xA5 are kept on both sides of the
+        workspace; `guards_intact()` tells whether any kernel wrote outside it."""
         _require_cuda()
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.opts = opts
@@ -173,10 +176,17 @@ class Solver:
         if nbytes == 0:
             raise GrmhdError("grmhd_workspace_bytes", EINVAL)
         self.workspace_bytes = int(nbytes)
+        gb = (int(guard_bytes) + 255) // 256 * 256
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            self._ws = torch.empty(nbytes + 256 + 2 * gb, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        base = (self._ws.data_ptr() + 255) // 256 * 256
+        base = (self._ws.data_ptr() + 255) // 256 * 256 + gb
+        self._guard = None
+        if gb:
+            off = base - self._ws.data_ptr()
+            self._guard = (self._ws[off - gb:off], self._ws[off + nbytes:off + nbytes + gb])
+            for t in self._guard:
+                t.fill_(0xA5)
         self.h = C.c_void_p()
         d = (C.c_double * 3)(*[float(x) for x in dx])
         rc = L.grmhd_create(self.nx, self.ny, self.nz, G, d, C.byref(opts), C.c_void_p(base),
@@ -184,6 +194,12 @@ class Solver:
                             C.byref(self.h))
         if rc != OK:
             raise GrmhdError("grmhd_create", rc)
+
+    def guards_intact(self) -> bool:
+        """True if the guard zones around the workspace still hold their pattern."""
+        assert self._guard is not None, "create the Solver with guard_bytes > 0"
+        self.stream.synchronize()
+        return all(bool((t == 0xA5).all()) for t in self._guard)
 
     def close(self):
         if getattr(self, "h", None) is not None and self.h.value:

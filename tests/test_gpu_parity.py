@@ -545,6 +545,77 @@ def test_source_kernels_are_bit_identical():
         a.close(); b.close()
 
 
+def _solver_with_guards(w, guard=1 << 20, **override):
+    from paper_2406_11669_b200 import binding
+    opts = dict(w.opts)
+    opts.update(override)
+    s = binding.Solver(w.nx, w.ny, w.nz, w.dx, binding.make_opts(**opts), guard_bytes=guard)
+    s.set_metric(w.metric)
+    s.set_prims(w.prims)
+    if w.vecpot is not None:
+        s.set_vecpot(w.vecpot)
+    if w.mask is not None:
+        s.set_mask(w.mask)
+    return s
+
+
+def test_no_kernel_writes_outside_the_workspace():
+    """compute-sanitizer is closed on this pool, so the out-of-bounds check is our own: 1 MiB of
+    0xA5 on both sides of the caller-owned workspace must survive every kernel family -- both flux
+    kernel families, both source kernels, flux-CT / upwind CT (both edge kernels), Lorenz gauge,
+    backup con2prim, RK2/3/4, eager and graph steps, host and device I/O -- on blocks that are
+    ragged in every direction, narrower than a tile, and one cell thick."""
+    cases = [(wl.c2p_stress(45), {}), (wl.kerr_blob(40), {"emf": 1}),
+             (wl.kerr_blob(40), {"emf": 1, "uct_passes": 0, "gauge": 1}),
+             (wl.bns_like(33), {"gauge": 1}), (wl.blast(44), {"flux_kernel": 0, "src_kernel": 0}),
+             (wl.c2p_stress(36), {"c2p_backup": 1, "graph": 0}), (wl.balsara1(256, 4, 4), {}),
+             (wl.balsara1(67, 5, 3), {"emf": 1}), (wl.alfven_wave(16, 1, 1, axis=0), {}),
+             (wl.alfven_wave(16, 1, 1, axis=0), {"emf": 1, "gauge": 1})]
+    for w, opt in cases:
+        g = _solver_with_guards(w)
+        for k, v in opt.items():
+            g.set_option(k, v)
+        assert g.guards_intact(), (w.name, opt, "after set_*")
+        g.step(4, w.cfl)            # eager, capture, graph replays
+        g.get_cons(); g.get_prims(); g.get_vecpot()
+        g.get_cons(host=True)
+        assert g.guards_intact(), (w.name, opt)
+        assert g.stats()["rc"] == 0
+        g.close()
+
+
+def test_repeated_runs_are_bit_identical():
+    """What a race in the shared-memory exchanges of the flux kernels, the TMA ring (slot reuse
+    across the async proxy), the staged source tile or the atomics of the reductions would break:
+    the same three steps from the same data, twelve times over on two handles, must give the same
+    bits every time (state, A_i, dt, max speeds, counters)."""
+    for w, opt in ((wl.c2p_stress(45), {}), (wl.kerr_blob(40), {"emf": 1, "gauge": 1}),
+                   (wl.bns_like(33), {}), (wl.blast(44), {"graph": 0})):
+        first = None
+        handles = [make_gpu(w), make_gpu(w)]
+        for g in handles:
+            for k, v in opt.items():
+                g.set_option(k, v)
+        for rep in range(6):
+            for g in handles:
+                g.set_prims(w.prims)
+                if w.vecpot is not None:
+                    g.set_vecpot(w.vecpot)
+                g.step(3, w.cfl)
+                st = g.stats()
+                state = to_np(g.get_cons()) + to_np(g.get_vecpot())
+                sig = (st["t"], st["dt"], tuple(st["maxspeed"]), st["c2p_fail"], st["p_fix"],
+                       st["atmo"], st["w_cap"])
+                if first is None:
+                    first = (state, sig)
+                    continue
+                assert sig == first[1], (w.name, opt, rep)
+                for x, y in zip(state, first[0]):
+                    assert np.array_equal(x, y), (w.name, opt, rep)
+        for g in handles:
+            g.close()
+
+
 def test_config1_full_run_to_t04():
     """Config 1 at full size and full length: same number of steps, same final state."""
     w = wl.balsara1(256, 4, 4)
