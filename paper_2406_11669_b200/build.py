@@ -29,7 +29,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         os.path.getmtime(LIB) < os.path.getmtime(p) for p in _deps())
     if force or stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        # GRMHD_NVCC_EXTRA: extra nvcc flags (e.g. "-DFT_NSLOTS=2") for tuning sweeps of the
+        # compile-time parameters the kernels expose
+        extra = os.environ.get("GRMHD_NVCC_EXTRA", "").split()
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.check_call(cmd)
     return LIB
