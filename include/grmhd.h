@@ -167,6 +167,10 @@ int grmhd_get_psi(grmhd* h, double* field);
  * narrower than 32 cells in x use anyway);
  * "src_kernel" (1 default: the metric-derivative stencils of the source terms in x and y from a
  * TMA-staged shared-memory tile; 0: plain loads -- bit-identical results);
+ * "small_fuse" (1 default: blocks of at most 2^16 padded cells, where a step is bound by kernel
+ * launches, run the x, y and z fluxes in one launch, the three ghost-fill passes of A_i in one
+ * launch of a thread-block cluster, and the source terms and t += dt inside the post-update
+ * kernel -- 11 instead of 26 launches per RK2 step; 0: the kernel sequence of large blocks);
  * "graph" (1 default: after one eager step the launch sequence of a step is captured into a
  * CUDA graph and every later step is one cudaGraphLaunch into the handle's stream -- same
  * kernels, same arguments, bit-identical results; any other option or grmhd_set_mask drops the

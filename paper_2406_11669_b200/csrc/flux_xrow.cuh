@@ -130,4 +130,28 @@ k_flux_xrow(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems,
   }
 }
 
+// The three directions in ONE launch (launch-bound small blocks): the items of x, then y, then z,
+// every pencil of each (mode 0 above); same per-item code, so the stored fluxes are bit-identical
+// to three k_flux_xrow launches.
+struct FluxAllArgs {
+  int nsd[3];          // segments per pencil
+  long long first[4];  // first item of direction d; first[3] = all items
+};
+template <int RECON, bool UCT>
+__global__ void __launch_bounds__(FX_THREADS, FX_MINB)
+k_flux_all(double* __restrict__ base, Geom g, Eos E, FluxAllArgs fa, int ap) {
+  const long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
+  if (item >= fa.first[3]) return;
+  const int d = item >= fa.first[2] ? 2 : (item >= fa.first[1] ? 1 : 0);
+  const long long it = item - fa.first[d];
+  const int nsd = fa.nsd[d];
+  const int seg = (int)(it % nsd);
+  const int row = (int)(it / nsd);
+  const int w0 = (d == 0 ? g.ny : g.nx) + 2 * ap;
+  const int t0 = row % w0 - ap, t1 = row / w0 - ap;
+  if (d == 0) fx_item<0, RECON, UCT>(base, g, E, seg * FX_VALID - 3, t0, t1, 0, g.nx + 1);
+  else if (d == 1) fx_item<1, RECON, UCT>(base, g, E, seg * FX_VALID - 3, t0, t1, 0, g.ny + 1);
+  else fx_item<2, RECON, UCT>(base, g, E, seg * FX_VALID - 3, t0, t1, 0, g.nz + 1);
+}
+
 }  // namespace gk

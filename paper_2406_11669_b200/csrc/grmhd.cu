@@ -45,6 +45,7 @@ struct grmhd {
   int uct_nseg = 16;     // segments of the marching passes along y and z
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
   int nsm = 148;         // multiprocessors of the device (queried at create)
+  int small_fuse = 1;    // 1: launch-bound blocks (<= SMALL_BLOCK_MAX padded cells) take the fused launches
   int flux_impl = 1;     // 1: y and z fluxes by k_flux_tma (blocks at least 32 cells wide in x),
                          // 0: k_flux_xrow (lanes along the flux direction) everywhere
   // CUDA graph of one RK step (launch-bound small blocks): the first step after a change of
@@ -255,6 +256,7 @@ int zero_field(grmhd* h, int id) {
 }
 
 // R15: x, then y, then z pass
+constexpr long long SMALL_BLOCK_MAX = 1LL << 16;  // padded cells: below, a step is launch bound
 constexpr long long FILL_FUSE_MAX = 1LL << 20;  // padded cells: below, launches cost more than threads
 
 int fill_ghosts(grmhd* h, const FillArgs& fa) {
@@ -265,6 +267,19 @@ int fill_ghosts(grmhd* h, const FillArgs& fa) {
   if (plain && npad <= FILL_FUSE_MAX) {
     k_fill_copy3<<<dim3((unsigned)((npad + 255) / 256), 1, fa.nf), 256, 0, h->s>>>(h->base, g, fa);
     CKL("k_fill_copy3");
+    return GRMHD_OK;
+  }
+  if (h->small_fuse && npad <= SMALL_BLOCK_MAX) {  // staggered / extrapolated fields, small block:
+    cudaLaunchConfig_t cfg = {};                    // the three passes by one cluster
+    cfg.gridDim = dim3(FILL1_CTAS);
+    cfg.blockDim = dim3(FILL1_THREADS);
+    cfg.stream = h->s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = FILL1_CTAS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    CK(cudaLaunchKernelEx(&cfg, k_fill_axes1, h->base, g, fa));
+    h->launches++;
     return GRMHD_OK;
   }
   for (int a = 0; a < 3; a++) {
@@ -306,6 +321,13 @@ int set_params(grmhd* h, double cfl, double t_end) {
 
 int launch_src(grmhd* h);
 
+// launch-bound blocks take fused launches: k_flux_all, k_fill_axes1, k_post with sources and t += dt
+bool small_block(const grmhd* h) {
+  const Geom& g = h->g;
+  return h->small_fuse &&
+         (long long)(g.nx + 2 * G) * (g.ny + 2 * G) * (g.nz + 2 * G) <= SMALL_BLOCK_MAX;
+}
+
 // R13 + R14 + R15 after a change of (U~, A)
 int after_stage(grmhd* h, bool want_speed) {
   const Geom& g = h->g;
@@ -314,19 +336,28 @@ int after_stage(grmhd* h, bool want_speed) {
     rc = fill_ghosts(h, fill_vecpot(h->E.gauge != 0));
     if (rc) return rc;
   });
+  const bool small = small_block(h);
+  // small blocks: the sources and the end-of-step t += dt ride in k_post (two launches fewer)
+  const int flags = (want_speed ? 1 : 0) | (small && want_speed ? 2 : 0);
+  const unsigned char* mk = h->have_mask ? h->mask : nullptr;
   KT(KG_C2P, {
-    if (h->E.c2p_backup)
-      k_post<false, true><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
-          h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+    const dim3 pg = grd_post(g), pb(32, KP_BY, KP_BZ);
+    if (small && h->E.c2p_backup)
+      k_post<false, true, true><<<pg, pb, 0, h->s>>>(h->base, mk, g, h->E, h->dst, flags);
+    else if (small)
+      k_post<false, false, true><<<pg, pb, 0, h->s>>>(h->base, mk, g, h->E, h->dst, flags);
+    else if (h->E.c2p_backup)
+      k_post<false, true><<<pg, pb, 0, h->s>>>(h->base, mk, g, h->E, h->dst, flags);
     else
-      k_post<false, false><<<grd_post(g), dim3(32, KP_BY, KP_BZ), 0, h->s>>>(
-          h->base, h->have_mask ? h->mask : nullptr, g, h->E, h->dst, want_speed ? 1 : 0);
+      k_post<false, false><<<pg, pb, 0, h->s>>>(h->base, mk, g, h->E, h->dst, flags);
     CKL("k_post");
   });
-  KT(KG_SRC, {
-    rc = launch_src(h);
-    if (rc) return rc;
-  });
+  if (!small) {
+    KT(KG_SRC, {
+      rc = launch_src(h);
+      if (rc) return rc;
+    });
+  }
   KT(KG_GHOST, {
     rc = fill_ghosts(h, fill_prims());
     if (rc) return rc;
@@ -501,8 +532,38 @@ int launch_flux_d(grmhd* h) {
   return GRMHD_OK;
 }
 
+// launch-bound small blocks: x, y and z in one launch (k_flux_all, lanes along the flux direction)
+template <int RECON>
+int launch_flux_all(grmhd* h) {
+  const Geom& g = h->g;
+  const int ap = apron_width(h);
+  FluxAllArgs fa;
+  fa.first[0] = 0;
+  for (int d = 0; d < 3; d++) {
+    fa.nsd[d] = (g.n(d) + 1 + FX_VALID - 1) / FX_VALID;
+    const int nt0 = d == 0 ? g.ny : g.nx, nt1 = d == 2 ? g.ny : g.nz;
+    fa.first[d + 1] = fa.first[d] + (long long)(nt0 + 2 * ap) * (nt1 + 2 * ap) * fa.nsd[d];
+  }
+  const long long nblk = (fa.first[3] + FX_THREADS / 32 - 1) / (FX_THREADS / 32);
+  if (h->E.emf)
+    k_flux_all<RECON, true><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, fa, ap);
+  else
+    k_flux_all<RECON, false><<<(unsigned)nblk, FX_THREADS, 0, h->s>>>(h->base, g, h->E, fa, ap);
+  CKL("k_flux_all");
+  return GRMHD_OK;
+}
+
 int compute_fluxes(grmhd* h) {
   int rc;
+  if (small_block(h)) {
+    const int recon = h->o.recon == 0 ? 0 : (h->o.ppm_flatten ? 2 : 1);
+    KT(KG_FLUX_X, {
+      rc = recon == 0 ? launch_flux_all<0>(h)
+                      : (recon == 1 ? launch_flux_all<1>(h) : launch_flux_all<2>(h));
+      if (rc) return rc;
+    });
+    return GRMHD_OK;
+  }
   KT(KG_FLUX_X, { if ((rc = launch_flux_d<0>(h))) return rc; });
   KT(KG_FLUX_Y, { if ((rc = launch_flux_d<1>(h))) return rc; });
   KT(KG_FLUX_Z, { if ((rc = launch_flux_d<2>(h))) return rc; });
@@ -569,10 +630,12 @@ int one_step_eager(grmhd* h) {
     rc = after_stage(h, s == ns - 1);
     if (rc) return rc;
   }
-  KT(KG_MISC, {
-    k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 1);
-    CKL("k_dt");
-  });
+  if (!small_block(h)) {  // (small blocks: t += dt is done by the last k_post)
+    KT(KG_MISC, {
+      k_dt<<<1, 1, 0, h->s>>>(h->dst, g, 1);
+      CKL("k_dt");
+    });
+  }
   h->steps++;
   return GRMHD_OK;
 }
@@ -912,6 +975,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "flux_kernel") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_kernel is 0 or 1");
     h->flux_impl = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "small_fuse") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: small_fuse is 0 or 1");
+    h->small_fuse = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "src_kernel") == 0) {

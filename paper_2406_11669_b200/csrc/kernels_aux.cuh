@@ -99,23 +99,20 @@ struct FillArgs {
   int nf;
 };
 
-__global__ void k_fill_axis(double* __restrict__ base, Geom g, FillArgs fa, int a) {
-  const int f = blockIdx.z;
-  if (f >= fa.nf) return;
+// one item of the pass along axis a: field f, transverse position tid (false: past the end)
+__device__ __forceinline__ bool fill_axis_item(double* __restrict__ base, const Geom& g,
+                                               const FillArgs& fa, int a, int f, long long tid) {
   double* q = fld(base, g, fa.id[f]);
   const int st = fa.stag[f], kind = fa.kind[f];
   const int b0 = (a + 1) % 3, b1 = (a + 2) % 3;
   const int lo0 = b0 < a ? -G : 0, hi0 = g.n(b0) - 1 + ((st >> b0) & 1) + (b0 < a ? G : 0);
   const int lo1 = b1 < a ? -G : 0, hi1 = g.n(b1) - 1 + ((st >> b1) & 1) + (b1 < a ? G : 0);
   const int n0 = hi0 - lo0 + 1, n1 = hi1 - lo1 + 1;
+  if (tid >= (long long)n0 * n1) return false;
   // make the x-like axis the fast thread index whenever it is transverse
   int t0, t1;
-  {
-    const long long tid = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (tid >= (long long)n0 * n1) return;
-    if (b0 == 0 || (b1 != 0 && b0 < b1)) { t0 = (int)(tid % n0); t1 = (int)(tid / n0); }
-    else { t1 = (int)(tid % n1); t0 = (int)(tid / n1); }
-  }
+  if (b0 == 0 || (b1 != 0 && b0 < b1)) { t0 = (int)(tid % n0); t1 = (int)(tid / n0); }
+  else { t1 = (int)(tid % n1); t0 = (int)(tid / n1); }
   int I[3];
   I[b0] = lo0 + t0; I[b1] = lo1 + t1;
   const int na = g.n(a), sa = (st >> a) & 1;
@@ -150,6 +147,32 @@ __global__ void k_fill_axis(double* __restrict__ base, Geom g, FillArgs fa, int 
       q[c0 + gl * sd] = v;
       q2 = q1; q1 = v;
     }
+  }
+  return true;
+}
+
+__global__ void k_fill_axis(double* __restrict__ base, Geom g, FillArgs fa, int a) {
+  const int f = blockIdx.z;
+  if (f >= fa.nf) return;
+  fill_axis_item(base, g, fa, a, f, blockIdx.x * (long long)blockDim.x + threadIdx.x);
+}
+
+// The x, y, z passes in ONE launch (launch-bound small blocks): one thread-block CLUSTER of
+// FILL1_CTAS blocks walks the items of a pass, then a cluster barrier (arrive.release /
+// wait.acquire: the global writes of every block of the cluster are ordered before the reads of
+// the next pass).  Same items, same arithmetic: bit-identical to three k_fill_axis launches.
+constexpr int FILL1_THREADS = 512;
+constexpr int FILL1_CTAS = 8;
+__global__ void __launch_bounds__(FILL1_THREADS) k_fill_axes1(double* __restrict__ base, Geom g,
+                                                               FillArgs fa) {
+  const int t0 = blockIdx.x * FILL1_THREADS + threadIdx.x;
+  for (int a = 0; a < 3; a++) {
+    const int b0 = (a + 1) % 3, b1 = (a + 2) % 3;
+    const long long nt = (long long)(g.n(b0) + 2 * G + 1) * (g.n(b1) + 2 * G + 1);
+    for (long long w = t0; w < nt * fa.nf; w += FILL1_THREADS * FILL1_CTAS)
+      fill_axis_item(base, g, fa, a, (int)(w / nt), w % nt);
+    asm volatile("barrier.cluster.arrive.release.aligned;\n"
+                 "barrier.cluster.wait.acquire.aligned;" ::: "memory");
   }
 }
 
@@ -355,10 +378,28 @@ constexpr int KP_THREADS = 32 * KP_BY * KP_BZ;
 #ifndef KP_MINB
 #define KP_MINB 5
 #endif
-template <bool INIT, bool BACKUP>
-__global__ void __launch_bounds__(KP_THREADS, KP_MINB)
+// The metric and U~ rows are first used after the stores of B~ and B_c, which the compiler cannot
+// move loads across (one workspace: it must assume aliasing): their lines are asked for at kernel
+// entry with prefetch.global.L2, at no register cost.  Measured at 256^3: 1.350 ms without,
+// 1.315 ms with (L1 instead of L2: 1.320 ms).
+#ifndef KP_PREFETCH
+#define KP_PREFETCH 1
+#endif
+__device__ __forceinline__ void kp_opaque(double& x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void kp_prefetch(const double* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+// SRC (launch-bound small blocks): also R9, the sources of the recovered primitives (otherwise
+// k_src / k_src_tile).  flags: bit 0 = accumulate the max speeds, bit 1 = end of a step, t += dt
+// (otherwise k_dt mode 1).
+template <bool INIT, bool BACKUP, bool SRC = false>
+__global__ void __launch_bounds__(KP_THREADS, SRC ? 1 : KP_MINB)
 k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g, Eos E,
-       DevState* __restrict__ st, int want_speed) {
+       DevState* __restrict__ st, int flags) {
+  const int want_speed = flags & 1;
+  if ((flags & 2) && blockIdx.x + blockIdx.y + blockIdx.z == 0 &&
+      threadIdx.x + threadIdx.y + threadIdx.z == 0)
+    st->t += st->dt;
   const int i = blockIdx.x * 32 + threadIdx.x - G;
   const int j = blockIdx.y * KP_BY + threadIdx.y - G;
   const int kraw = blockIdx.z * KP_BZ + threadIdx.z - G;
@@ -369,6 +410,14 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
   double Bx = 0.0, By = 0.0, Bz = 0.0;
   Met M;
   double sg = 1.0;
+#if KP_PREFETCH
+  if (!INIT && (threadIdx.x & 15) == 0) {  // one request per 128-byte line (c is clamped: valid)
+#pragma unroll
+    for (int f = 0; f < 10; f++) kp_prefetch(fld(base, g, F_MET + f) + c);
+#pragma unroll
+    for (int r = 0; r < 5; r++) kp_prefetch(fld(base, g, F_Y + r) + c);
+  }
+#endif
   if (inpad) {
     const double* Ax = fld(base, g, F_Y + 5);
     const double* Ay = fld(base, g, F_Y + 6);
@@ -426,6 +475,25 @@ k_post(double* __restrict__ base, const unsigned char* __restrict__ mask, Geom g
     }
     const Prim P = {P5[0], P5[1], P5[2], P5[3], P5[4], Bx, By, Bz};
     if (want_speed) cell_speeds(P, M, E, s);
+    if (SRC) {
+      // The inputs pass through an opaque barrier: without it the compiler shares sub-expressions
+      // (point_state, det gamma, gamma^ij) with con2prim / prim2con above and contracts other
+      // products into FMAs than in the stand-alone k_src -- the results then differ in the last
+      // bit.  With it cell_sources is compiled as in k_src: bit-identical.
+      Prim Ps = P;
+      Met Ms = M;
+      double sgs = sg;
+      kp_opaque(Ps.rho); kp_opaque(Ps.vx); kp_opaque(Ps.vy); kp_opaque(Ps.vz); kp_opaque(Ps.p);
+      kp_opaque(Ps.Bx); kp_opaque(Ps.By); kp_opaque(Ps.Bz);
+      kp_opaque(Ms.a); kp_opaque(Ms.bx); kp_opaque(Ms.by); kp_opaque(Ms.bz);
+      kp_opaque(Ms.gxx); kp_opaque(Ms.gxy); kp_opaque(Ms.gxz);
+      kp_opaque(Ms.gyy); kp_opaque(Ms.gyz); kp_opaque(Ms.gzz);
+      kp_opaque(sgs);
+      double S[4];
+      cell_sources(base, g, c, Ps, Ms, sgs, E, S);
+#pragma unroll
+      for (int r = 0; r < 4; r++) fld(base, g, F_SRC + r)[c] = S[r];
+    }
   }
   if (!INIT) {
     // counters: integer sums and maxima, order independent
