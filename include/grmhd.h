@@ -165,6 +165,11 @@ int grmhd_get_psi(grmhd* h, double* field);
  * "flux_kernel" (1 default: y and z fluxes by the TMA-fed marching kernel, x fluxes with the lanes
  * of a warp along x; 0: lanes along the flux direction in all three directions -- what blocks
  * narrower than 32 cells in x use anyway);
+ * "flux_xcol" (1 default: with flux-CT the two apron columns x = -1 and x = nx of the y and z
+ * fluxes are computed from compact, contiguous copies of those columns -- the static face metric
+ * copied once per grmhd_set_metric, the primitives and B once per substep -- and only the flux row
+ * flux-CT reads there is stored; 0: straight from the padded arrays, where consecutive cells of a
+ * column are a row pitch apart -- bit-identical results);
  * "src_kernel" (1 default: the metric-derivative stencils of the source terms in x and y from a
  * TMA-staged shared-memory tile; 0: plain loads -- bit-identical results);
  * "small_fuse" (1 default: blocks of at most 2^16 padded cells, where a step is bound by kernel

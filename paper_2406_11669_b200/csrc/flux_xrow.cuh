@@ -48,28 +48,88 @@ __device__ __forceinline__ void fx_recon(double q, double qm1, double qp1, doubl
   }
 }
 
+// Where an item's data live.  FxPadded: the padded [field][z][y][x] arrays of the workspace.
+struct FxPadded {
+  const double* base;
+  long long NPA;
+  static constexpr bool compact = false;
+  template <int D>
+  __device__ __forceinline__ int index(const Geom& g, int cc, int t0, int t1) const {
+    return (int)(D == 0 ? g.at(cc, t0, t1) : (D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc)));
+  }
+  __device__ __forceinline__ double load(int field, int idx) const {
+    return base[(size_t)field * NPA + idx];
+  }
+};
+
+// FxXcol: the COMPACT COPIES of the two x-apron columns x = -1 (side 0) and x = nx (side 1).
+// In the padded arrays consecutive cells of such a column are a row pitch apart: one useful
+// double per DRAM atom.  k_xcol_gather copies the columns of the XC_NSLOT fields an apron face
+// needs into [slot][side][z][y] arrays (y fastest) in one spare field of the workspace -- the 22
+// static face-metric fields once per grmhd_set_metric, the 10 dynamic ones once per substep for
+// both the y and the z fluxes -- and the apron faces are then computed from contiguous data.
+constexpr int XC_NSLOT = 32;
+__host__ __device__ constexpr int xc_slot(int field) {
+  // P 0-4, B_c 5-7, B~^y 8, B~^z 9, static face metric of y 10-20, of z 21-31
+  return field >= F_FM + 2 * NFM ? 21 + (field - F_FM - 2 * NFM)
+       : field >= F_FM + NFM     ? 10 + (field - F_FM - NFM)
+       : field >= F_BF           ? 8 + (field - F_BF - 1)
+       : field >= F_BC           ? 5 + (field - F_BC)
+                                 : field - F_P;
+}
+__host__ __device__ constexpr int xc_field(int slot) {
+  return slot < 5 ? F_P + slot : slot < 8 ? F_BC + slot - 5 : slot < 10 ? F_BF + 1 + slot - 8
+       : slot < 21 ? F_FM + NFM + slot - 10 : F_FM + 2 * NFM + slot - 21;
+}
+struct FxXcol {
+  const double* xc;  // the spare field
+  int PY, PZ;
+  static constexpr bool compact = true;
+  // pencils of direction y: (t0, t1) = (x, z), lanes along y; of direction z: (x, y), along z
+  template <int D>
+  __device__ __forceinline__ int index(const Geom& g, int cc, int t0, int t1) const {
+    const int side = t0 < 0 ? 0 : 1;
+    const int jj = (D == 1 ? cc : t1) + G, kk = (D == 1 ? t1 : cc) + G;
+    return (side * PZ + kk) * PY + jj;
+  }
+  __device__ __forceinline__ double load(int field, int idx) const {
+    return xc[(size_t)xc_slot(field) * 2 * PZ * PY + idx];
+  }
+};
+
+// columns of the slots [s0, s0 + gridDim.z / 2) -> compact; blockIdx.z = 2 (slot - s0) + side
+__global__ void k_xcol_gather(double* __restrict__ base, Geom g, long long xc_off, int s0) {
+  const int jj = blockIdx.x * blockDim.x + threadIdx.x;
+  const int kk = blockIdx.y * blockDim.y + threadIdx.y;
+  if (jj >= g.PY || kk >= g.PZ) return;
+  const int slot = s0 + (int)(blockIdx.z >> 1), side = (int)(blockIdx.z & 1);
+  const int x = side ? g.nx + X0 : X0 - 1;
+  const double v = base[(size_t)xc_field(slot) * g.NPA + (long long)kk * g.sz + (long long)jj * g.sy + x];
+  base[xc_off + ((size_t)(slot * 2 + side) * g.PZ + kk) * g.PY + jj] = v;
+}
+
 // One item: the warp's 32 lanes are the cells c0 .. c0+31 along D of the pencil (t0, t1) -- with
 // (t0, t1) the transverse axes: (y, z) for D = x, (x, z) for D = y, (x, y) for D = z -- and the
 // lane of cell c solves face c - 1/2.  Faces outside [flo, fhi) are not stored.  Call with whole
 // warps.  UCT (compile time): also store the upwind-CT face rows of F_W.
-template <int D, int RECON, bool UCT>
-__device__ __forceinline__ void fx_item(double* __restrict__ base, const Geom& g, const Eos& E,
-                                        int c0, int t0, int t1, int flo, int fhi) {
+template <int D, int RECON, bool UCT, class AD>
+__device__ __forceinline__ void fx_item_at(double* __restrict__ base, const Geom& g, const Eos& E,
+                                           const AD& ad, int c0, int t0, int t1, int flo, int fhi) {
   const int lane = threadIdx.x & 31;
   const int nD = g.n(D);
   const int c = c0 + lane;                  // this lane's cell along D; its face is c - 1/2
   const int cc = min(c, nD + G - 1);        // lanes past the last ghost cell reuse it
-  const int idx = (int)(D == 0 ? g.at(cc, t0, t1) : (D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc)));
+  const int idx = ad.template index<D>(g, cc, t0, t1);
 
   // ---- cell data of the lane: rho, v^x, v^y, v^z, p and the two transverse B; the static face
   // metric and the staggered normal field of the lane's face c - 1/2
   double q[FX_NV];
 #pragma unroll
-  for (int v = 0; v < FX_NV; v++) q[v] = fld(base, g, flux_var_field(D, v))[idx];
-  const double bfx = fld(base, g, F_BF + D)[idx];
+  for (int v = 0; v < FX_NV; v++) q[v] = ad.load(flux_var_field(D, v), idx);
+  const double bfx = ad.load(F_BF + D, idx);
   double mv11[NFM];
 #pragma unroll
-  for (int v = 0; v < NFM; v++) mv11[v] = fld(base, g, F_FM + NFM * D + v)[idx];
+  for (int v = 0; v < NFM; v++) mv11[v] = ad.load(F_FM + NFM * D + v, idx);
   // ---- neighbours across lanes
   double qm1[FX_NV], qp1[FX_NV];
 #pragma unroll
@@ -93,7 +153,16 @@ __device__ __forceinline__ void fx_item(double* __restrict__ base, const Geom& g
   const FaceMet fmet = face_met<D>(mv11);
   double out[7], w[4];
   ft_face<D, UCT>(qL, qR, bfx, fmet, E, out, w);
-  if (lane >= 3 && lane < 3 + FX_VALID && c >= flo && c < fhi) {
+  if constexpr (AD::compact) {
+    // x-apron columns: flux-CT (R10) reads there only the row of B~^x -- F~y(B~x) is row 6 of the
+    // y fluxes, F~z(B~x) row 5 of the z fluxes (k_update) -- stored at its place in the padded array
+    static_assert(D != 0 && !UCT, "compact columns: y / z fluxes with flux-CT");
+    if (lane >= 3 && lane < 3 + FX_VALID && c >= flo && c < fhi) {
+      const long long pidx = D == 1 ? g.at(t0, cc, t1) : g.at(t0, t1, cc);
+      constexpr int row = D == 1 ? 6 : 5;
+      fld(base, g, flux_field(D) + row)[pidx] = out[row];
+    }
+  } else if (lane >= 3 && lane < 3 + FX_VALID && c >= flo && c < fhi) {
     double* o = fld(base, g, flux_field(D)) + idx;
     const size_t NPA = (size_t)g.NPA;
 #pragma unroll
@@ -104,6 +173,28 @@ __device__ __forceinline__ void fx_item(double* __restrict__ base, const Geom& g
       for (int r = 0; r < 4; r++) ow[r * NPA] = w[r];
     }
   }
+}
+
+template <int D, int RECON, bool UCT>
+__device__ __forceinline__ void fx_item(double* __restrict__ base, const Geom& g, const Eos& E,
+                                        int c0, int t0, int t1, int flo, int fhi) {
+  const FxPadded ad = {base, g.NPA};
+  fx_item_at<D, RECON, UCT>(base, g, E, ad, c0, t0, t1, flo, fhi);
+}
+
+// The 2 x-apron columns of the y or z fluxes (flux-CT) from the compact column copies: one warp
+// per (column, t1, segment) item as mode 1 of k_flux_xrow with ap = 1; same per-face code.
+template <int D, int RECON>
+__global__ void __launch_bounds__(FX_THREADS, FX_MINB)
+k_flux_xcol(double* __restrict__ base, Geom g, Eos E, int nsd, long long nitems, long long xc_off) {
+  const long long item = (long long)blockIdx.x * (FX_THREADS / 32) + (threadIdx.x >> 5);
+  if (item >= nitems) return;  // warp uniform
+  const int seg = (int)(item % nsd);
+  const int row = (int)(item / nsd);
+  const int q0 = row % 2, t1 = row / 2 - 1;
+  const int t0 = q0 == 0 ? -1 : g.nx;
+  const FxXcol ad = {base + xc_off, g.PY, g.PZ};
+  fx_item_at<D, RECON, false>(base, g, E, ad, seg * FX_VALID - 3, t0, t1, 0, g.n(D) + 1);
 }
 
 // grid: one warp per (pencil, segment) item: item = pencil * nsd + seg.  `ap` = the transverse

@@ -45,6 +45,7 @@ struct grmhd {
   int uct_nseg = 16;     // segments of the marching passes along y and z
   int uct_passes = 1;    // upwind CT: per-axis passes (1) or the per-edge kernel k_emf_uct (0)
   int nsm = 148;         // multiprocessors of the device (queried at create)
+  int xcol = 1;          // 1: x-apron columns of the y/z fluxes from compact column copies
   int small_fuse = 1;    // 1: launch-bound blocks (<= SMALL_BLOCK_MAX padded cells) take the fused launches
   int flux_impl = 1;     // 1: y and z fluxes by k_flux_tma (blocks at least 32 cells wide in x),
                          // 0: k_flux_xrow (lanes along the flux direction) everywhere
@@ -188,7 +189,8 @@ long long stage_elems_of(const Geom& g) {
   return ((n + 31) / 32) * 32;
 }
 
-int nfields_of(const grmhd_opts* o) { return o->rk == 4 ? F_END_RK4 : F_END_RK23; }
+// the fields of layout.cuh + one spare field: the compact x-apron columns (FxXcol, flux_xrow.cuh)
+int nfields_of(const grmhd_opts* o) { return (o->rk == 4 ? F_END_RK4 : F_END_RK23) + 1; }
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes at;
@@ -449,6 +451,34 @@ int launch_src(grmhd* h) {
   return GRMHD_OK;
 }
 
+// ---- compact x-apron columns (FxXcol, flux_xrow.cuh) ----------------------------------------
+long long xc_offset(const grmhd* h) { return (long long)(h->nfields - 1) * h->g.NPA; }
+// usable when the TMA-fed kernels serve y and z (so the aprons are a launch of their own), with
+// flux-CT (one apron column per side, one flux row needed), and the 32 column pairs fit the field
+bool xcol_ok(const grmhd* h) {
+  const Geom& g = h->g;
+  return h->xcol && h->flux_impl == 1 && h->tma_ok && g.nx >= 32 &&
+         (long long)XC_NSLOT * 2 * g.PY * g.PZ <= g.NPA;
+}
+int xcol_gather(grmhd* h, int s0, int ns) {
+  const Geom& g = h->g;
+  k_xcol_gather<<<dim3((g.PY + 31) / 32, (g.PZ + 3) / 4, 2 * ns), dim3(32, 4, 1), 0, h->s>>>(
+      h->base, g, xc_offset(h), s0);
+  CKL("k_xcol_gather");
+  return GRMHD_OK;
+}
+template <int D, int RECON>
+int launch_flux_xcol(grmhd* h) {
+  const Geom& g = h->g;
+  const int nsd = (g.n(D) + 1 + FX_VALID - 1) / FX_VALID;
+  const int nt1 = D == 2 ? g.ny : g.nz;
+  const long long nitems = 2LL * (nt1 + 2) * nsd;
+  k_flux_xcol<D, RECON><<<(unsigned)((nitems + FX_THREADS / 32 - 1) / (FX_THREADS / 32)),
+                          FX_THREADS, 0, h->s>>>(h->base, g, h->E, nsd, nitems, xc_offset(h));
+  CKL("k_flux_xcol");
+  return GRMHD_OK;
+}
+
 template <int D, int RECON, bool UCT>
 int launch_flux_tma_v(grmhd* h) {
   const Geom& g = h->g;
@@ -489,6 +519,11 @@ int launch_flux_tma_v(grmhd* h) {
   // the 2 ap apron columns along x.  (Run beside the main kernel on a second stream they cost
   // MORE, measured 0.93 against 0.89 ms: their blocks take register space the main kernel's
   // third block per SM needs.)
+  if constexpr (!UCT) {
+    // ... unless the columns have compact copies (gathered once per substep in compute_fluxes):
+    // contiguous loads, and only the one row flux-CT reads there is stored
+    if (xcol_ok(h)) return launch_flux_xcol<D, RECON>(h);
+  }
   return launch_flux_xrow<D, RECON>(h, 1, h->s);
 }
 
@@ -565,7 +600,11 @@ int compute_fluxes(grmhd* h) {
     return GRMHD_OK;
   }
   KT(KG_FLUX_X, { if ((rc = launch_flux_d<0>(h))) return rc; });
-  KT(KG_FLUX_Y, { if ((rc = launch_flux_d<1>(h))) return rc; });
+  KT(KG_FLUX_Y, {
+    // the dynamic x-apron columns (P, B_c, B~^y, B~^z) for the y AND the z fluxes
+    if (!h->E.emf && xcol_ok(h) && (rc = xcol_gather(h, 0, 10))) return rc;
+    if ((rc = launch_flux_d<1>(h))) return rc;
+  });
   KT(KG_FLUX_Z, { if ((rc = launch_flux_d<2>(h))) return rc; });
   return GRMHD_OK;
 }
@@ -794,6 +833,12 @@ int grmhd_set_metric(grmhd* h, const double* const field[16]) {
   CKL("k_face_metric");
   k_face_metric<2><<<fg, fb, 0, h->s>>>(h->base, h->g);
   CKL("k_face_metric");
+  // compact copies of the x-apron columns of the static y and z face metric (slots 10 .. 31);
+  // always kept up to date where they fit, whatever the options say now
+  if ((long long)XC_NSLOT * 2 * h->g.PY * h->g.PZ <= h->g.NPA) {
+    int rc = xcol_gather(h, 10, 22);
+    if (rc) return rc;
+  }
   h->have_metric = true;
   // a new metric under existing primitives: U~, B_c, the sources and the max speed are rebuilt
   // from the primitives by the next call that needs them
@@ -980,6 +1025,11 @@ int grmhd_set_option(grmhd* h, const char* key, double value) {
   if (std::strcmp(key, "small_fuse") == 0) {
     if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: small_fuse is 0 or 1");
     h->small_fuse = (int)value;
+    return GRMHD_OK;
+  }
+  if (std::strcmp(key, "flux_xcol") == 0) {
+    if (value != 0.0 && value != 1.0) return fail(h, GRMHD_EINVAL, "set_option: flux_xcol is 0 or 1");
+    h->xcol = (int)value;
     return GRMHD_OK;
   }
   if (std::strcmp(key, "src_kernel") == 0) {

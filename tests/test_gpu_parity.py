@@ -545,6 +545,37 @@ def test_source_kernels_are_bit_identical():
         a.close(); b.close()
 
 
+def test_compact_apron_columns_are_bit_identical():
+    """The x-apron columns of the y and z fluxes computed from compact column copies
+    ("flux_xcol" = 1: gathered static face metric, per-substep gather of P, B_c, B~, one stored
+    flux row) against the same faces straight from the padded arrays ("flux_xcol" = 0): same
+    per-face code, so everything flux-CT makes of them -- A_i, B, the conserved state, the
+    primitives incl. ghosts -- has identical bits; outflow and periodic, with mask, RK2/3/4,
+    ragged blocks, a second set_metric on a live handle, and the options that bypass it."""
+    cases = [(wl.kerr_blob(40), {}), (wl.c2p_stress(45), {}), (wl.bns_like(33), {}),
+             (wl.blast(44), {}), (wl.balsara1(256, 4, 4), {"small_fuse": 0}),
+             (wl.blast(44), {"gauge": 1}), (wl.kerr_blob(40), {"emf": 1})]
+    for w, opt in cases:
+        a, b = make_gpu(w), make_gpu(w)
+        b.set_option("flux_xcol", 0)
+        for k, v in opt.items():
+            a.set_option(k, v); b.set_option(k, v)
+        for rep in range(2):
+            a.step(3, w.cfl)
+            b.step(3, w.cfl)
+            names = ["U%d" % r for r in range(8)] + ["A%d" % r for r in range(3)] + ["P%d" % r for r in range(8)]
+            for nm, x, y in zip(names,
+                                to_np(a.get_cons()) + to_np(a.get_vecpot()) + to_np(a.get_prims()),
+                                to_np(b.get_cons()) + to_np(b.get_vecpot()) + to_np(b.get_prims())):
+                assert np.array_equal(x, y), (w.name, opt, rep, nm, float(np.abs(x - y).max()))
+            sa, sb = a.stats(), b.stats()
+            assert sa["dt"] == sb["dt"] and sa["t"] == sb["t"]
+            # the same metric again on the live handles: the static column copies are regathered
+            for s_ in (a, b):
+                s_.set_metric(w.metric)
+        a.close(); b.close()
+
+
 def test_small_block_fused_launches_are_bit_identical():
     """Launch-bound blocks (<= 2^16 padded cells) take fused launches -- x/y/z fluxes in one
     (k_flux_all), the three ghost-fill passes of A_i in one cluster launch (k_fill_axes1), the
@@ -599,7 +630,7 @@ def test_no_kernel_writes_outside_the_workspace():
     ragged in every direction, narrower than a tile, and one cell thick."""
     cases = [(wl.c2p_stress(45), {}), (wl.kerr_blob(40), {"emf": 1}),
              (wl.kerr_blob(40), {"emf": 1, "uct_passes": 0, "gauge": 1}),
-             (wl.bns_like(33), {"gauge": 1}), (wl.blast(44), {"flux_kernel": 0, "src_kernel": 0}),
+             (wl.bns_like(33), {"gauge": 1}), (wl.blast(44), {"flux_kernel": 0, "src_kernel": 0}), (wl.blast(44), {"flux_xcol": 0}),
              (wl.c2p_stress(36), {"c2p_backup": 1, "graph": 0}), (wl.balsara1(256, 4, 4), {}),
              (wl.balsara1(67, 5, 3), {"emf": 1}), (wl.balsara1(67, 5, 3), {"small_fuse": 0}),
              (wl.alfven_wave(16, 1, 1, axis=0), {}),
