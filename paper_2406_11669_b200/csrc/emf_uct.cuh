@@ -118,6 +118,9 @@ __device__ __forceinline__ int uct_vbar_field(int a, int b) {  // vbar^a on the 
 #ifndef UM_MINB
 #define UM_MINB 6
 #endif
+#ifndef UM_CHUNK
+#define UM_CHUNK 2
+#endif
 template <int A>
 __global__ void __launch_bounds__(128, UM_MINB)
 k_uct_march(double* __restrict__ base, Geom g, int seglen, int wr, int fin,
@@ -152,37 +155,44 @@ k_uct_march(double* __restrict__ base, Geom g, int seglen, int wr, int fin,
     mv[v].step(q[v][(m0 + 1) * sA], 0.0, false, qm, qp);  // position m0 - 1
     mv[v].qpp = qp;
   }
-  // values of the next step, loaded one step ahead
-  double nq[2], na[4];
-  auto fetch = [&](int m) {
-    const long long c = m * sA;
-    nq[0] = q[0][c + 2 * sA]; nq[1] = q[1][c + 2 * sA];
-    na[0] = Ap[c]; na[1] = Ap[c - sb]; na[2] = Am[c]; na[3] = Am[c - sb];
-  };
-  fetch(m0);
-  for (int m = m0; m < m1; m++) {
-    const double cq0 = nq[0], cq1 = nq[1];
-    const double ap = ft_max(na[0], na[1]), am = ft_max(na[2], na[3]);
-    if (m + 1 < m1) fetch(m + 1);
-    double L[2], R[2];
-    {
-      double qm, qp;
-      mv[0].step(cq0, 0.0, false, qm, qp);
-      L[0] = mv[0].qpp; R[0] = qm; mv[0].qpp = qp;  // q^+ of position m-1, q^- of position m
-      mv[1].step(cq1, 0.0, false, qm, qp);
-      L[1] = mv[1].qpp; R[1] = qm; mv[1].qpp = qp;
+  // The march is serial along A, so its loads are what can overlap: the inputs of a chunk of
+  // UM_CHUNK steps (2 reconstructed values, 4 a+- values and the pending first bracket each) are
+  // all requested before the first of them is used.
+  const int need_e = !first;
+  for (int mb = m0; mb < m1; mb += UM_CHUNK) {
+    double cq[UM_CHUNK][2], ca[UM_CHUNK][4], ce[UM_CHUNK];
+#pragma unroll
+    for (int u = 0; u < UM_CHUNK; u++) {
+      const long long c = (long long)min(mb + u, m1 - 1) * sA;  // the tail repeats its last step
+      cq[u][0] = q[0][c + 2 * sA]; cq[u][1] = q[1][c + 2 * sA];
+      ca[u][0] = Ap[c]; ca[u][1] = Ap[c - sb]; ca[u][2] = Am[c]; ca[u][3] = Am[c - sb];
+      ce[u] = need_e ? Ec[c] : 0.0;
     }
-    const long long c = m * sA;
-    const double br = sign * uct_combine(ap, am, L[0], R[0], L[1], R[1]);
-    const double e = first ? br : Ec[c] + br;
-    if (last) {
-      if (ok) {
-        double rhs = -e;
-        if (gauge) rhs -= (GA[c + sc] - GA[c]) * g.idx[comp];
-        rk_apply(base, g, 5 + comp, c0 + c, rhs, h, rk);
+#pragma unroll
+    for (int u = 0; u < UM_CHUNK; u++) {
+      const int m = mb + u;
+      if (m >= m1) break;
+      const double ap = ft_max(ca[u][0], ca[u][1]), am = ft_max(ca[u][2], ca[u][3]);
+      double L[2], R[2];
+      {
+        double qm, qp;
+        mv[0].step(cq[u][0], 0.0, false, qm, qp);
+        L[0] = mv[0].qpp; R[0] = qm; mv[0].qpp = qp;  // q^+ of position m-1, q^- of position m
+        mv[1].step(cq[u][1], 0.0, false, qm, qp);
+        L[1] = mv[1].qpp; R[1] = qm; mv[1].qpp = qp;
       }
-    } else {
-      Ec[c] = e;
+      const long long c = m * sA;
+      const double br = sign * uct_combine(ap, am, L[0], R[0], L[1], R[1]);
+      const double e = first ? br : ce[u] + br;
+      if (last) {
+        if (ok) {
+          double rhs = -e;
+          if (gauge) rhs -= (GA[c + sc] - GA[c]) * g.idx[comp];
+          rk_apply(base, g, 5 + comp, c0 + c, rhs, h, rk);
+        }
+      } else {
+        Ec[c] = e;
+      }
     }
   }
 }
