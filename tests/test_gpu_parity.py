@@ -473,9 +473,12 @@ def test_bns_100_substeps_smooth():
     ("kerr", 100, 1e-9, 0.0),        # smooth accretion blob: 4.4e-11 measured, counters identical
     ("blast", 200, 0.1, 2e-3),       # strong shock + 1 % pressure fixes: 1.7e-2 measured
     ("stress", 20, None, 1e-2),      # leaves the recovery's domain (1.9 M failures): counters only
+    ("bns", 50, 1e-9, 0.0),          # config 5's own length (RK4 x 50) at 32^3, SURVEY 8(d) (ii):
+                                     # 7.6e-11 measured, 281 481 pressure fixes on both sides
 ])
 def test_full_length_runs_at_64_cubed(name, nsteps, drift_bound, count_rtol):
-    w = {"kerr": wl.kerr_blob, "blast": wl.blast, "stress": wl.c2p_stress}[name](64)
+    w = wl.bns_like(32) if name == "bns" else \
+        {"kerr": wl.kerr_blob, "blast": wl.blast, "stress": wl.c2p_stress}[name](64)
     r, g = make_ref(w), make_gpu(w)
     r.step(nsteps, w.cfl)
     g.step(nsteps, w.cfl)
