@@ -555,9 +555,12 @@ def test_compact_apron_columns_are_bit_identical():
     per-face code, so everything flux-CT makes of them -- A_i, B, the conserved state, the
     primitives incl. ghosts -- has identical bits; outflow and periodic, with mask, RK2/3/4,
     ragged blocks, a second set_metric on a live handle, and the options that bypass it."""
-    cases = [(wl.kerr_blob(40), {}), (wl.c2p_stress(45), {}), (wl.bns_like(33), {}),
-             (wl.blast(44), {}), (wl.balsara1(256, 4, 4), {"small_fuse": 0}),
-             (wl.blast(44), {"gauge": 1}), (wl.kerr_blob(40), {"emf": 1})]
+    # the compact copies need nx >= 56 (32 column pairs must fit one field); narrower blocks and
+    # the upwind CT fall back to the padded-array launch -- both kinds are here
+    cases = [(wl.kerr_blob(72), {}), (wl.c2p_stress(61), {}), (wl.bns_like(57), {}),
+             (wl.blast(64), {}), (wl.balsara1(256, 4, 4), {"small_fuse": 0}),
+             (wl.balsara1(97, 6, 5), {"small_fuse": 0}), (wl.blast(64), {"gauge": 1}),
+             (wl.kerr_blob(72), {"emf": 1}), (wl.kerr_blob(40), {}), (wl.c2p_stress(45), {})]
     for w, opt in cases:
         a, b = make_gpu(w), make_gpu(w)
         b.set_option("flux_xcol", 0)
@@ -631,7 +634,8 @@ def test_no_kernel_writes_outside_the_workspace():
     kernel families, both source kernels, flux-CT / upwind CT (both edge kernels), Lorenz gauge,
     backup con2prim, RK2/3/4, eager and graph steps, host and device I/O -- on blocks that are
     ragged in every direction, narrower than a tile, and one cell thick."""
-    cases = [(wl.c2p_stress(45), {}), (wl.kerr_blob(40), {"emf": 1}),
+    cases = [(wl.c2p_stress(45), {}), (wl.c2p_stress(61), {}), (wl.kerr_blob(72), {"gauge": 1}),
+             (wl.kerr_blob(40), {"emf": 1}),
              (wl.kerr_blob(40), {"emf": 1, "uct_passes": 0, "gauge": 1}),
              (wl.bns_like(33), {"gauge": 1}), (wl.blast(44), {"flux_kernel": 0, "src_kernel": 0}), (wl.blast(44), {"flux_xcol": 0}),
              (wl.c2p_stress(36), {"c2p_backup": 1, "graph": 0}), (wl.balsara1(256, 4, 4), {}),
@@ -657,7 +661,7 @@ def test_repeated_runs_are_bit_identical():
     the same three steps from the same data, twelve times over on two handles, must give the same
     bits every time (state, A_i, dt, max speeds, counters)."""
     for w, opt in ((wl.c2p_stress(45), {}), (wl.kerr_blob(40), {"emf": 1, "gauge": 1}),
-                   (wl.bns_like(33), {}), (wl.blast(44), {"graph": 0})):
+                   (wl.bns_like(33), {}), (wl.blast(44), {"graph": 0}), (wl.c2p_stress(61), {})):
         first = None
         handles = [make_gpu(w), make_gpu(w)]
         for g in handles:
