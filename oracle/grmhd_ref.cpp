@@ -13,9 +13,14 @@
 // P6 curl/div/flux-CT identities, P7 HLLE consistency, P8 reconstruction properties,
 // P9 speeds closed forms, P10 con2prim closed forms, P11 sources vs brute-force 4-D
 // Christoffels, P12 naive re-evaluation on 4^3 blocks, P13 constant-metric advection,
-// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45), P16 upwind CT (eqs 33-35), P17 the generalised Lorenz gauge (eqs 31-32).  Parity UNPINNED by the paper: the PPM variant (G8)
-// and the characteristic-speed bound (G9) are readings of citations that are not in
-// PAPER.md; they are pinned only by the mathematical properties P8/P9.
+// P14 Rindler hydrostatic equilibrium, P15 the 1-D backup con2prim (eqs 42-45), P16 upwind CT
+// (eqs 33-35), P17 the generalised Lorenz gauge (eqs 31-32); and by hand-worked numbers
+// (tests/test_oracle_pins2.py): R16 max speed / dt / step_until clipping, R12 temporal order
+// 2 / 3 / 4 of the RK tableaux, R15 linear continuation of A_i, R5 face floors and velocity cap,
+// G16 static face field on a varying metric, G8(c) flattening between its ends, R7 HLLE.
+// Parity UNPINNED by the paper: the PPM variant (G8) and the characteristic-speed bound (G9)
+// are readings of citations that are not in PAPER.md; they are pinned only by the
+// mathematical properties P8/P9.
 #include "grmhd_ref.h"
 
 #include <algorithm>
