@@ -223,16 +223,8 @@ k_flux_tma(double* __restrict__ base, Geom g, Eos E, int seglen, int ngx, int ap
       const int slot = n % FT_SLOTS;
       ft_mbar_wait(&sm.bar[slot], (unsigned)((n / FT_SLOTS) & 1));
       double mv11[NFM];
-#ifdef FT_DIRECT
-      {
-        const double* mg = fld(base, g, F_FM + NFM * D) + ublk + plB + (F + clB) * sd;
-#pragma unroll
-        for (int v = 0; v < NFM; v++) mv11[v] = mg[v * NPA];
-      }
-#else
 #pragma unroll
       for (int v = 0; v < NFM; v++) mv11[v] = sm.fm[slot][v * MF + ringo];
-#endif
       const FaceMet fmet = face_met<D>(mv11);
       const double bfn = sm.bf[slot][ringo];
       double qL[FX_NV], qR[FX_NV];
