@@ -17,7 +17,8 @@
 // (eqs 33-35), P17 the generalised Lorenz gauge (eqs 31-32); and by hand-worked numbers
 // (tests/test_oracle_pins2.py): R16 max speed / dt / step_until clipping, R12 temporal order
 // 2 / 3 / 4 of the RK tableaux, R15 linear continuation of A_i, R5 face floors and velocity cap,
-// G16 static face field on a varying metric, G8(c) flattening between its ends, R7 HLLE.
+// G16 static face field on a varying metric, G8(c) flattening between its ends, R7 HLLE,
+// F2 Lax-Friedrichs (eq. 30).
 // Parity UNPINNED by the paper: the PPM variant (G8) and the characteristic-speed bound (G9)
 // are readings of citations that are not in PAPER.md; they are pinned only by the
 // mathematical properties P8/P9.

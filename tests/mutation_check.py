@@ -34,6 +34,10 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("LxF: sign of the dissipation term", "Fhat[r] = 0.5 * (GR + GL - cw * (UR[r] - UL[r]));", "Fhat[r] = 0.5 * (GR + GL + cw * (UR[r] - UL[r]));"),
+ ("LxF: c_wave = min", "const double cw = std::max(cmax, cmin);", "const double cw = std::min(cmax, cmin);"),
+ ("LxF: c_wave = c_max alone", "const double cw = std::max(cmax, cmin);", "const double cw = cmax;"),
+ ("LxF: missing 1/2 on the dissipation", "Fhat[r] = 0.5 * (GR + GL - cw * (UR[r] - UL[r]));", "Fhat[r] = 0.5 * (GR + GL) - cw * (UR[r] - UL[r]);"),
  ("HLLE: cmax/cmin swapped on the fluxes", "Fhat[r] = (cmin * GR + cmax * GL - cmax * cmin * (UR[r] - UL[r])) / (cmax + cmin);", "Fhat[r] = (cmax * GR + cmin * GL - cmax * cmin * (UR[r] - UL[r])) / (cmax + cmin);"),
 ]
 res={}

@@ -318,3 +318,75 @@ def test_R7_hlle_worked_number():
     got = ref.riemann_pt(0, np.array([1.0, 0.9, 0, 0, 0.01, 0, 0, 0]),
                          np.array([1.0, 0.9, 0, 0, 0.01, 0, 0, 0]), flat, o)
     np.testing.assert_allclose(got[[0, 1, 4]], FL, rtol=1e-14)
+
+
+# ------------------------------------------------------------ F2: Lax-Friedrichs, eq. (30)
+def test_F2_lxf_worked_number():
+    """eq. (30) (PAPER.md:202-206): F = [F_r + F_l - c_wave (U_r - U_l)] / 2 with c_wave =
+    max(c_max, c_min), on flat-space B = 0 Riemann problems with every ingredient from the textbook
+    special-relativistic formulas in numpy (as test_R7_hlle_worked_number): no oracle point
+    function enters the expected value.  The mistakes it exists to catch: the sign of the
+    dissipation term, c_wave = min or c_max alone, a missing 1/2, U and F swapped."""
+    Gam = 1.4
+    o = ref.make_opts(gamma_ad=Gam, rho_atm=1e-12, p_floor=1e-30, riemann=1)
+    flat = np.array([1.0, 0, 0, 0, 1.0, 0, 0, 1.0, 0, 1.0])
+
+    def side(rho, v, p):
+        W = 1.0 / np.sqrt(1.0 - v * v)
+        h = 1.0 + Gam / (Gam - 1.0) * p / rho
+        D, S = rho * W, rho * h * W * W * v
+        tau = rho * h * W * W - p - D
+        cs = np.sqrt(Gam * p / (rho * h))
+        return (np.array([D, S, tau]), np.array([D * v, S * v + p, S - D * v]),
+                (v - cs) / (1.0 - v * cs), (v + cs) / (1.0 + v * cs))
+
+    # (left state, right state): in the first c_max > c_min, in the second (both flows to the
+    # left) c_min > c_max, so that max(c_max, c_min) is told apart from either of its arguments
+    for (rl, vl, pl), (rr, vr, pr) in (((1.0, 0.4, 1.0), (0.3, -0.2, 0.2)),
+                                       ((0.5, -0.6, 0.3), (1.2, -0.3, 0.8))):
+        UL, FL, lmL, lpL = side(rl, vl, pl)
+        UR, FR, lmR, lpR = side(rr, vr, pr)
+        cmax, cmin = max(0.0, lpL, lpR), -min(0.0, lmL, lmR)
+        assert abs(cmax - cmin) > 0.05
+        want = 0.5 * (FR + FL - max(cmax, cmin) * (UR - UL))
+        got = ref.riemann_pt(0, np.array([rl, vl, 0, 0, pl, 0, 0, 0]),
+                             np.array([rr, vr, 0, 0, pr, 0, 0, 0]), flat, o)
+        np.testing.assert_allclose(got[[0, 1, 4]], want, rtol=1e-14)
+        assert np.all(got[[2, 3, 5, 6, 7]] == 0.0)
+        # and it is NOT the HLLE flux of the same states (the option is honoured)
+        hlle = ref.riemann_pt(0, np.array([rl, vl, 0, 0, pl, 0, 0, 0]),
+                              np.array([rr, vr, 0, 0, pr, 0, 0, 0]), flat,
+                              ref.make_opts(gamma_ad=Gam, rho_atm=1e-12, p_floor=1e-30, riemann=0))
+        assert np.abs(hlle[[0, 1, 4]] - want).max() > 1e-3
+    # consistency: equal states give the physical flux, whatever c_wave is
+    UL, FL, _, _ = side(0.7, 0.25, 0.4)
+    P = np.array([0.7, 0.25, 0, 0, 0.4, 0, 0, 0])
+    np.testing.assert_allclose(ref.riemann_pt(0, P, P, flat, o)[[0, 1, 4]], FL, rtol=1e-14)
+
+
+def test_F2_lxf_is_more_dissipative_than_hlle_on_a_block():
+    """PAPER.md:206 ("more dissipative than HLLE"): an entropy wave (uniform v and p, sinusoidal
+    rho) advected on a periodic flat block keeps its amplitude exactly; both schemes lose some,
+    the LxF run more; both conserve the total rest mass to round-off (eq. 30 is a conservative
+    flux)."""
+    n = 16
+    x = (np.arange(n) + 0.5) / n
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    one = np.ones_like(X)
+    prim = [1.0 + 0.2 * np.sin(2 * np.pi * X), 0.3 * one, 0 * one, 0 * one, one, 0 * one, 0 * one,
+            0 * one]
+    prim = [wl.wrap_pad(q) for q in prim]
+    metric = wl.flat_metric(prim[0].shape)
+    amps, mass = {}, {}
+    for riemann in (0, 1):
+        o = dict(OPTS); o.update(riemann=riemann, recon=0, rk=2, bc=(0, 0, 0))
+        s_ = ref.RefSolver(n, n, n, (1.0 / n,) * 3, ref.make_opts(**o))
+        s_.set_metric(metric); s_.set_prims(prim)
+        D0 = interior(s_.get_cons()[0]).copy()
+        s_.step(20, 0.25)
+        D1 = interior(s_.get_cons()[0])
+        amps[riemann] = (D1.max() - D1.min()) / (D0.max() - D0.min())
+        mass[riemann] = abs(D1.sum() - D0.sum()) / D0.sum()
+    assert amps[1] < amps[0] < 1.0, amps
+    assert amps[0] - amps[1] > 1e-3, amps
+    assert mass[0] < 1e-13 and mass[1] < 1e-13, mass
