@@ -34,6 +34,9 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("mask: i and k swapped", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G)];", "h->mask[h->idx(i, j, k)] = mask[((size_t)(std::min(i, h->nz - 1) + G) * sy + (j + G)) * sx + (std::min(k, h->nx - 1) + G)];"),
+ ("mask: shifted by one cell in x", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G)];", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G - 1)];"),
+ ("mask: ignored by con2prim", "const int bits = con2prim(Uin, B, M, o, have_mask && mask[c], P5, U5, &it,", "const int bits = con2prim(Uin, B, M, o, false, P5, U5, &it,"),
  ("LxF: sign of the dissipation term", "Fhat[r] = 0.5 * (GR + GL - cw * (UR[r] - UL[r]));", "Fhat[r] = 0.5 * (GR + GL + cw * (UR[r] - UL[r]));"),
  ("LxF: c_wave = min", "const double cw = std::max(cmax, cmin);", "const double cw = std::min(cmax, cmin);"),
  ("LxF: c_wave = c_max alone", "const double cw = std::max(cmax, cmin);", "const double cw = cmax;"),

@@ -257,6 +257,25 @@ def test_minmod_lxf_rk2_variants():
         _one_step_case(w2)
 
 
+def test_asymmetric_mask_on_a_non_cubic_block():
+    """set_mask: config 3's own mask is a sphere on a cubic grid, symmetric under every index
+    permutation -- here three marked cells with pairwise different indices on non-cubic blocks
+    (narrow: lanes-along-D kernels; wide: TMA kernels and the compact apron columns), so that a
+    transposed or shifted index in k_repack_mask cannot pass; counters must agree exactly."""
+    for base in (wl.balsara1(41, 6, 5), wl.balsara1(70, 9, 6)):
+        shape = (base.nz + 6, base.ny + 6, base.nx + 6)
+        mask = np.zeros(shape, dtype=np.uint8)
+        for i, j, k in ((1, 2, 3), (base.nx - 2, 0, 4), (base.nx // 2, base.ny - 1, 0)):
+            mask[k + 3, j + 3, i + 3] = 1
+        mask[0, 0, 0] = 1                     # a ghost cell: ignored
+        w = wl.Workload(**{**base.__dict__, "mask": mask, "name": base.name + "_asym_mask"})
+        _one_step_case(w, nsteps=2)
+        r, g = make_ref(w), make_gpu(w)
+        r.step(2, w.cfl); g.step(2, w.cfl)
+        assert g.stats()["atmo"] == r.stats()["atmo"] == 3 * w.stages * 2
+        g.close()
+
+
 def test_tiny_and_degenerate_blocks():
     """1-cell-thick periodic blocks and the smallest outflow block."""
     _one_step_case(wl.alfven_wave(16, 1, 1, axis=0), nsteps=3)

@@ -390,3 +390,41 @@ def test_F2_lxf_is_more_dissipative_than_hlle_on_a_block():
     assert amps[1] < amps[0] < 1.0, amps
     assert amps[0] - amps[1] > 1e-3, amps
     assert mass[0] < 1e-13 and mass[1] < 1e-13, mass
+
+
+# ------------------------------------------------ mask: the right cells, on every substep
+def test_mask_marks_the_right_cells_on_every_substep():
+    """`set_mask` (excised region, config 3): the cells given as mask[k+G, j+G, i+G] != 0 -- and
+    only those -- are reset to the atmosphere on EVERY substep (G20), on a non-cubic block with an
+    asymmetric mask, so that a transposed or shifted index, a mask applied once per step only, or
+    one that also eats its neighbours cannot pass (config 3's own mask is a sphere on a cubic
+    grid: symmetric under every index permutation)."""
+    nx, ny, nz = 9, 7, 5
+    shape = (nz + 2 * G, ny + 2 * G, nx + 2 * G)
+    o = dict(OPTS); o.update(rk=3, bc=(1, 1, 1), rho_atm=1e-7)
+    met = const_fields(shape, [1.0, 0, 0, 0, 1, 0, 0, 1, 0, 1, 0, 0, 0, 0, 0, 0])
+    prim = const_fields(shape, [1.0, 0.1, -0.05, 0.02, 0.5, 0.01, 0.02, -0.01])
+    marked = [(1, 2, 3), (7, 0, 4), (4, 6, 0)]            # (i, j, k), all different in every index
+    mask = np.zeros(shape, dtype=np.uint8)
+    for i, j, k in marked:
+        mask[k + G, j + G, i + G] = 1
+    mask[0, 0, 0] = 1                                      # a ghost cell: must be ignored
+    s = ref.RefSolver(nx, ny, nz, (0.1, 0.1, 0.1), ref.make_opts(**o))
+    s.set_metric(met); s.set_prims(prim); s.set_mask(mask)
+    nsteps = 2
+    s.step(nsteps, 0.2)
+    P = s.get_prims()
+    rho = interior(P[0])
+    is_atmo = np.zeros((nz, ny, nx), dtype=bool)
+    for i, j, k in marked:
+        is_atmo[k, j, i] = True
+    assert np.all(rho[is_atmo] == 1e-7)
+    assert np.all(interior(P[1])[is_atmo] == 0.0) and np.all(interior(P[3])[is_atmo] == 0.0)
+    assert np.all(rho[~is_atmo] > 0.5), "only the marked cells are reset"
+    st = s.stats()
+    assert st["atmo"] == len(marked) * 3 * nsteps, st["atmo"]   # every substep of every step
+    # without the mask nothing is reset
+    s2 = ref.RefSolver(nx, ny, nz, (0.1, 0.1, 0.1), ref.make_opts(**o))
+    s2.set_metric(met); s2.set_prims(prim)
+    s2.step(nsteps, 0.2)
+    assert s2.stats()["atmo"] == 0 and np.all(interior(s2.get_prims()[0]) > 0.5)
