@@ -34,6 +34,9 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("ghost fill: mirror instead of copy", "          src = (kind == 0) ? 0 : g + 1;", "          src = (kind == 0) ? -g - 1 : g + 1;"),
+ ("ghost fill: upper side copies the wrong layer", "          src = (kind == 0) ? hi[a] : g - 1;", "          src = (kind == 0) ? hi[a] - 1 : g - 1;"),
+ ("ghost fill: corners left out", "      lo[a] = glo; hi[a] = ghi;\n    }\n  }", "    }\n  }"),
  ("mask: i and k swapped", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G)];", "h->mask[h->idx(i, j, k)] = mask[((size_t)(std::min(i, h->nz - 1) + G) * sy + (j + G)) * sx + (std::min(k, h->nx - 1) + G)];"),
  ("mask: shifted by one cell in x", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G)];", "h->mask[h->idx(i, j, k)] = mask[((size_t)(k + G) * sy + (j + G)) * sx + (i + G - 1)];"),
  ("mask: ignored by con2prim", "const int bits = con2prim(Uin, B, M, o, have_mask && mask[c], P5, U5, &it,", "const int bits = con2prim(Uin, B, M, o, false, P5, U5, &it,"),

@@ -428,3 +428,39 @@ def test_mask_marks_the_right_cells_on_every_substep():
     s2.set_metric(met); s2.set_prims(prim)
     s2.step(nsteps, 0.2)
     assert s2.stats()["atmo"] == 0 and np.all(interior(s2.get_prims()[0]) > 0.5)
+
+
+# -------------------------------------------- R15 / A1: ghost fill of the primitives
+@pytest.mark.parametrize("bc", [(1, 1, 1), (0, 0, 0), (0, 1, 0), (1, 0, 1)])
+def test_R15_ghost_fill_of_the_primitives(bc):
+    """Row A1: after set_prims the three ghost layers of rho, v^i, p hold, on a
+    periodic axis, the wrapped interior value (period n) and, on an outflow axis, the value of the
+    nearest interior cell -- faces, edges and corners alike (x, then y, then z pass).  Expected
+    values by a numpy index map (wrap / clamp per axis), the caller's ghost values being junk.
+    Catches: a mirror instead of a copy, a wrap with period n + 1, a pass that leaves the corners
+    unfilled, periodic and outflow confused."""
+    nx, ny, nz = 7, 5, 4
+    rng = np.random.default_rng(3)
+    shape = (nz + 2 * G, ny + 2 * G, nx + 2 * G)
+    met = const_fields(shape, [1.0, 0, 0, 0, 1, 0, 0, 1, 0, 1, 0, 0, 0, 0, 0, 0])
+    inner = [rng.uniform(0.5, 1.5, (nz, ny, nx)), rng.uniform(-0.2, 0.2, (nz, ny, nx)),
+             rng.uniform(-0.2, 0.2, (nz, ny, nx)), rng.uniform(-0.2, 0.2, (nz, ny, nx)),
+             rng.uniform(0.5, 1.5, (nz, ny, nx))]
+    prim = []
+    for q in inner:
+        a = np.full(shape, 123.456)            # junk in the caller's ghost cells
+        a[I3] = q
+        prim.append(a)
+    prim += [np.zeros(shape)] * 3
+    o = dict(OPTS); o.update(bc=bc)
+    s = ref.RefSolver(nx, ny, nz, (0.1, 0.1, 0.1), ref.make_opts(**o))
+    s.set_metric(met); s.set_prims(prim)
+    P = s.get_prims()
+
+    def index_map(n, periodic):
+        i = np.arange(-G, n + G)
+        return i % n if periodic else np.clip(i, 0, n - 1)
+    ix, iy, iz = (index_map(n, b == 0) for n, b in zip((nx, ny, nz), bc))
+    for f in range(5):
+        want = inner[f][np.ix_(iz, iy, ix)]
+        assert np.array_equal(P[f], want), (bc, f)
