@@ -34,6 +34,16 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("audit: PPM interface coefficient 1/8", "qp = 0.5 * (q[2] + q[3]) - (dm_p - dm_0) / 6.0;  // q_{i+1/2}", "qp = 0.5 * (q[2] + q[3]) - (dm_p - dm_0) / 8.0;  // q_{i+1/2}"),
+ ("audit: PPM MC slope limit 1x instead of 2x", "std::min(2.0 * std::fabs(dp), 2.0 * std::fabs(dm))", "std::min(1.0 * std::fabs(dp), 1.0 * std::fabs(dm))"),
+ ("audit: PPM monotonisation overshoot fix on the wrong side", "if (D * m > D * D / 6.0) qm = 3.0 * q0 - 2.0 * qp;", "if (D * m > D * D / 6.0) qp = 3.0 * q0 - 2.0 * qm;"),
+ ("audit: minmod takes the larger slope", "  const double m = std::min(std::fabs(a), std::fabs(b));\n  return a > 0.0 ? m : -m;", "  const double m = std::max(std::fabs(a), std::fabs(b));\n  return a > 0.0 ? m : -m;"),
+ ("audit: eq 18 magnetic pressure b^2 instead of b^2/2", "  const double ptot = P[4] + 0.5 * s.b2;\n  F[0]", "  const double ptot = P[4] + 1.0 * s.b2;\n  F[0]"),
+ ("audit: eq 18 induction flux sign", "F[5 + k] = B[k] * vt[d] / M.alpha - B[d] * vt[k] / M.alpha;", "F[5 + k] = B[k] * vt[d] / M.alpha + B[d] * vt[k] / M.alpha;"),
+ ("audit: eq 18 tau flux without the alpha b^0 B^d/W term", "F[4] = U[4] * vt[d] / M.alpha + ptot * v[d] - s.ab0 * B[d] / s.W;", "F[4] = U[4] * vt[d] / M.alpha + ptot * v[d];"),
+ ("audit: eq 22 tau without the (alpha b^0)^2 term", "U[4] = (s.rhoh + s.b2) * W2 - (P[4] + 0.5 * s.b2) - sq(s.ab0) - U[0];", "U[4] = (s.rhoh + s.b2) * W2 - (P[4] + 0.5 * s.b2) - U[0];"),
+ ("audit: eq 13 b^2 without the (alpha b^0)^2 term", "s.b2 = (s.B2 + sq(s.ab0)) / sq(s.W);", "s.b2 = (s.B2) / sq(s.W);"),
+ ("audit: speeds with v_A^2 = b^2/rho h", "const double va2 = s.b2 / (s.rhoh + s.b2);", "const double va2 = s.b2 / (s.rhoh);"),
  ("ghost fill: mirror instead of copy", "          src = (kind == 0) ? 0 : g + 1;", "          src = (kind == 0) ? -g - 1 : g + 1;"),
  ("ghost fill: upper side copies the wrong layer", "          src = (kind == 0) ? hi[a] : g - 1;", "          src = (kind == 0) ? hi[a] - 1 : g - 1;"),
  ("ghost fill: corners left out", "      lo[a] = glo; hi[a] = ghi;\n    }\n  }", "    }\n  }"),
