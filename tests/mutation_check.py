@@ -34,6 +34,14 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("audit2: face metric by the 2-point mean", "m[f] = (-met[f][c0] + 9.0 * met[f][c1] + 9.0 * met[f][c2] - met[f][c3]) / 16.0;", "m[f] = 0.5 * (met[f][c1] + met[f][c2]);"),
+ ("audit2: metric derivative 2nd order", "return (8.0 * (p1 - m1) - (p2 - m2)) / (12.0 * dx[a]);", "return (p1 - m1) / (2.0 * dx[a]);"),
+ ("audit2: flux-CT E_z with the wrong neighbour", "            const double Ez = 0.25 * (-FxBy[idx(i, j - 1, k)] - FxBy[c] +\n                                      FyBx[idx(i - 1, j, k)] + FyBx[c]);", "            const double Ez = 0.25 * (-FxBy[idx(i - 1, j, k)] - FxBy[c] +\n                                      FyBx[idx(i, j - 1, k)] + FyBx[c]);"),
+ ("audit2: flux-CT E_y sign", "            kA[1][c] = -Ey;", "            kA[1][c] = Ey;"),
+ ("audit2: S_tau K term without the factor 2 on beta K", "t0 += T0i[i] * (2.0 * bK - dalpha[i]);", "t0 += T0i[i] * (bK - dalpha[i]);"),
+ ("audit2: B_c from the lower face only", "Bc[1][c] = 0.5 * (Bf[1][c] + Bf[1][idx(i, j + 1, k)]) / sg;", "Bc[1][c] = Bf[1][c] / sg;"),
+ ("audit2: Lorenz damping without alpha", "kPsi[c] = -div - xi * vertex(i, j, k).alpha * Psi[c];", "kPsi[c] = -div - xi * Psi[c];"),
+ ("audit2: UCT bracket dissipation sign", "  return (ap * vL * BL + am * vR * BR - ap * am * (BR - BL)) / (ap + am);", "  return (ap * vL * BL + am * vR * BR + ap * am * (BR - BL)) / (ap + am);"),
  ("audit: PPM interface coefficient 1/8", "qp = 0.5 * (q[2] + q[3]) - (dm_p - dm_0) / 6.0;  // q_{i+1/2}", "qp = 0.5 * (q[2] + q[3]) - (dm_p - dm_0) / 8.0;  // q_{i+1/2}"),
  ("audit: PPM MC slope limit 1x instead of 2x", "std::min(2.0 * std::fabs(dp), 2.0 * std::fabs(dm))", "std::min(1.0 * std::fabs(dp), 1.0 * std::fabs(dm))"),
  ("audit: PPM monotonisation overshoot fix on the wrong side", "if (D * m > D * D / 6.0) qm = 3.0 * q0 - 2.0 * qp;", "if (D * m > D * D / 6.0) qp = 3.0 * q0 - 2.0 * qm;"),

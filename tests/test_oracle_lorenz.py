@@ -86,3 +86,36 @@ def test_P17_damping_of_psi():
         s.step(6, 0.25)
     pd, pu = np.abs(s_d.get_psi()).max(), np.abs(s_u.get_psi()).max()
     assert 0 < pd < 0.7 * pu
+
+
+def test_P17_damping_term_carries_the_lapse():
+    """eqs (28), (32): d_t Psi = -d_j F_Psi^j - xi ALPHA Psi.  With a constant
+    lapse alpha = 0.8 (flat gamma, no shift) and Psi != 0 after a few steps, the oracle's d_t Psi is
+    compared with -d_j(alpha A_j) - (lorenz_xi/dt) alpha Psi formed in numpy from the A_i and Psi it
+    returns (vertex means and centred vertex differences as in test_P17_rhs_terms_against_numpy).
+    Catches the damping term without its lapse (test_P17_damping_of_psi runs with alpha = 1) and
+    the flux without it."""
+    n = 8
+    alpha = 0.8
+    w = _with_vecpot(smooth_periodic_workload(n, seed=4, curved=False))
+    w.metric[0] = np.full_like(w.metric[0], alpha)
+    s = make_ref(w)
+    s.set_option("gauge", 1.0)
+    s.set_option("lorenz_xi", 1.5)
+    s.step(3, 0.25)
+    dt = s.stats()["dt"]
+    _, dPsi = s.rhs_gauge()
+    I = slice(G, G + n)
+    A = [a[I, I, I] for a in s.get_vecpot()]
+    Psi = s.get_psi()[I, I, I]
+    assert np.abs(Psi).max() > 1e-6
+    dx = w.dx[0]
+    Av = [0.5 * (A[0] + np.roll(A[0], 1, 2)), 0.5 * (A[1] + np.roll(A[1], 1, 1)),
+          0.5 * (A[2] + np.roll(A[2], 1, 0))]
+    div = sum((np.roll(alpha * Av[d], -1, ax) - np.roll(alpha * Av[d], 1, ax)) / (2 * dx)
+              for d, ax in ((0, 2), (1, 1), (2, 0)))
+    want = -div - (1.5 / dt) * alpha * Psi
+    scale = np.abs(want).max()
+    assert np.abs(dPsi[I, I, I] - want).max() < 1e-12 * max(scale, 1.0)
+    # the two terms are told apart: without the lapse on the damping the answer moves by far more
+    assert np.abs((1.5 / dt) * (1.0 - alpha) * Psi).max() > 1e-6 * max(scale, 1.0)
