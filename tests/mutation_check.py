@@ -34,6 +34,12 @@ M=[
  ("flatten: threshold 0.5", "std::fabs(dp1) > 0.33 * std::min(p[3], p[1])", "std::fabs(dp1) > 0.5 * std::min(p[3], p[1])"),
  ("flatten: velocity test flipped", "&& vm1 > vp1) {", "&& vm1 < vp1) {"),
  ("c2p1d: t^2/x as printed", "0.5 * (t * t / (x * x) + s * iw2)", "0.5 * (t * t / x + s * iw2)"),
+ ("audit3: eq 41d without 1/Gamma", "eps = (z / (rho * W * W) - 1.0) / Gamma;", "eps = (z / (rho * W * W) - 1.0);"),
+ ("audit3: eq 40b with +B^2/2 (1 - v^2)", "const double f2 = tau + D - 0.5 * B2 * (1.0 + v2) + BS2 / (2.0 * z2) - z + p;", "const double f2 = tau + D - 0.5 * B2 * (1.0 - v2) + BS2 / (2.0 * z2) - z + p;"),
+ ("audit3: W cap rescales by f^2", "    for (int i = 0; i < 3; i++) v[i] *= f;\n    bits |= 8;", "    for (int i = 0; i < 3; i++) v[i] *= f * f;\n    bits |= 8;"),
+ ("equivalent (no test can tell: rho and v are kept, so the recomputed D = rho W is the D that came in): pressure fix also resets D", "    if (bits & 8) U5[0] = U[0];  // the pressure fix alone leaves D untouched", "    U5[0] = U[0];"),
+ ("audit3: undensitise in the step forgotten", "for (int r = 0; r < 5; r++) Uin[r] = U[r][c] / sg;  // undensitise, eq. (17)", "for (int r = 0; r < 5; r++) Uin[r] = U[r][c];"),
+ ("audit3: get_cons returns the densitised variables", "tmp[c] = r < 5 ? h->U[r][c] / h->sqrtg_cell(c) : h->Bc[r - 5][c];", "tmp[c] = r < 5 ? h->U[r][c] : h->Bc[r - 5][c];"),
  ("audit2: face metric by the 2-point mean", "m[f] = (-met[f][c0] + 9.0 * met[f][c1] + 9.0 * met[f][c2] - met[f][c3]) / 16.0;", "m[f] = 0.5 * (met[f][c1] + met[f][c2]);"),
  ("audit2: metric derivative 2nd order", "return (8.0 * (p1 - m1) - (p2 - m2)) / (12.0 * dx[a]);", "return (p1 - m1) / (2.0 * dx[a]);"),
  ("audit2: flux-CT E_z with the wrong neighbour", "            const double Ez = 0.25 * (-FxBy[idx(i, j - 1, k)] - FxBy[c] +\n                                      FyBx[idx(i - 1, j, k)] + FyBx[c]);", "            const double Ez = 0.25 * (-FxBy[idx(i - 1, j, k)] - FxBy[c] +\n                                      FyBx[idx(i, j - 1, k)] + FyBx[c]);"),
@@ -77,6 +83,6 @@ for name,a,b in M:
     failed=[l.split(" ")[1] for l in p.stdout.splitlines() if l.startswith("FAILED")]
     res[name]=failed; print(name,"->",failed,flush=True)
 open(cpp,"w").write(orig)
-holes=[k for k,v in res.items() if not v]
+holes=[k for k,v in res.items() if not v and not k.startswith("equivalent")]
 print("holes:", holes)
 sys.exit(1 if holes else 0)

@@ -464,3 +464,28 @@ def test_R15_ghost_fill_of_the_primitives(bc):
     for f in range(5):
         want = inner[f][np.ix_(iz, iy, ix)]
         assert np.array_equal(P[f], want), (bc, f)
+
+
+# ------------------------------------------------ eq. (17): densitised inside, plain outside
+def test_get_cons_is_undensitised_and_the_state_is_densitised():
+    """eq. (17): the evolved variables are sqrt(gamma) U, the ABI's get_cons
+    returns U itself (include/grmhd.h: 'UNdensitised D, S_x, S_y, S_z, tau').  On a constant
+    metric with sqrt(gamma) = 2 (gamma = diag(4, 1, 1), alpha = 0.9) and a fluid at rest the
+    closed forms are D = rho, S_j = 0, tau = rho eps + B_i B^i / 2 -- not twice that -- while the
+    conserved total the block carries, sum sqrt(gamma) D, is twice sum rho."""
+    nx, ny, nz = 6, 5, 4
+    shape = (nz + 2 * G, ny + 2 * G, nx + 2 * G)
+    met = const_fields(shape, [0.9, 0, 0, 0, 4.0, 0, 0, 1.0, 0, 1.0, 0, 0, 0, 0, 0, 0])
+    rho, p, B = 1.3, 0.7, (0.2, -0.3, 0.1)
+    prim = const_fields(shape, [rho, 0, 0, 0, p, *B])
+    o = dict(OPTS); o.update(bc=(0, 0, 0))
+    s = ref.RefSolver(nx, ny, nz, (0.1, 0.1, 0.1), ref.make_opts(**o))
+    s.set_metric(met); s.set_prims(prim)
+    U = s.get_cons()
+    B2 = 4.0 * B[0] ** 2 + B[1] ** 2 + B[2] ** 2            # B_i B^i with gamma_xx = 4
+    np.testing.assert_allclose(interior(U[0]), rho, rtol=1e-14)
+    for r in (1, 2, 3):
+        assert np.abs(interior(U[r])).max() < 1e-15
+    np.testing.assert_allclose(interior(U[4]), p / (G53 - 1.0) + 0.5 * B2, rtol=1e-13)
+    for d in range(3):
+        np.testing.assert_allclose(interior(U[5 + d]), B[d], rtol=1e-13)
